@@ -1,0 +1,186 @@
+/*
+ * cetra.h -- C ABI of the B200-native CETRA hot path (arXiv 2503.20875).
+ *
+ * Citations are line numbers of PAPER.md (the paper's text); "R<n>" are the readings of the
+ * paper listed in DESIGN.md.  The library implements, as hand-written sm_100a CUDA kernels:
+ *
+ *   linear search   (Eq. 1-2): for every trial duration D_j and every trial
+ *                   mid-transit time t_i, the weighted least-squares amplitude of the nearest-
+ *                   neighbour sampled transit template in the window [t_i - D_j/2, t_i + D_j/2]:
+ *                   depth, depth variance and the log-likelihood gain over the flat model;
+ *   periodic search (Eq. 3-4): phase-fold those per-(t_i, D_j) statistics over
+ *                   trial periods with nearest-neighbour lookup on the t0 grid, common depth,
+ *                   and reduce every period to its maximum-likelihood (t0, duration) element.
+ *
+ * Conventions (all entry points)
+ *  - Every function returns a cetra_status, never throws, never exits, allocates no device memory:
+ *    the caller owns every buffer and supplies the scratch workspace (size from the
+ *    *_workspace_bytes functions, 256-byte aligned).  Work is enqueued on `cuda_stream`
+ *    (a cudaStream_t passed as void*) and the call returns without synchronising unless stated.
+ *  - "_dev" pointers are device memory, "_host" pointers are host memory (pageable is fine) and are
+ *    free to be reused as soon as the call returns.
+ *  - The light curve is on a regular time grid (R1): the library checks
+ *    max_n |times[n] - times[0] - n*c| <= 1e-3*c with c = (times[n-1]-times[0])/(n-1), else
+ *    CETRA_ERR_NONUNIFORM_TIMES.  Null points (gaps, padding) are marked by a non-finite flux or a
+ *    non-finite / non-positive flux_err.  flux is normalised to baseline 1;
+ *    internally f = 1 - flux (R7).
+ *  - The t0 grid is t_i = t0_start + i*t0_stride, i < n_t0.  t0_start must lie on the
+ *    sample grid and t0_stride must be a whole number of cadences (else CETRA_ERR_UNSUPPORTED);
+ *    t0_start may lie before times[0] or t_i after times[n-1]: windows are clipped to the data (R9).
+ *  - Grids are stored [n_dur][n_t0], t0 contiguous, float32.  Cells whose window holds no
+ *    observation are NaN in all three grids.
+ *  - Arithmetic: FP32 products and sums on the CUDA cores, FP64 for every
+ *    quantity that decides an integer (template index R3, epoch cell R11).
+ */
+#ifndef CETRA_H_
+#define CETRA_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    CETRA_OK = 0,
+    CETRA_ERR_INVALID_ARG = -1,       /* null pointer, non-positive size, duration <= 0, period < t0_stride ... */
+    CETRA_ERR_NONUNIFORM_TIMES = -2,  /* times[] is not a regular grid */
+    CETRA_ERR_UNSUPPORTED = -3,       /* t0 grid off the sample grid, too many durations, index overflow */
+    CETRA_ERR_WORKSPACE = -4,         /* workspace null, misaligned or smaller than *_workspace_bytes */
+    CETRA_ERR_CUDA = -5               /* a CUDA runtime call failed (cudaGetLastError is left set) */
+} cetra_status;
+
+typedef enum { CETRA_F32 = 0, CETRA_F64 = 1 } cetra_dtype;
+
+#define CETRA_MAX_DURATIONS 128
+
+/* Uniform grid of trial mid-transit times. */
+typedef struct {
+    double t0_start;    /* days, same origin as times[] */
+    double t0_stride;   /* days, > 0 */
+    int64_t n_t0;       /* number of cells I */
+} cetra_t0_grid;
+
+/* One record of the periodogram: the maximum-likelihood element of one trial
+ * period.  A period with no candidate has lr = depth = depth_var = t0 = NaN and indices -1. */
+typedef struct {
+    float lr;           /* log-likelihood gain of the periodic model over the flat model (Eq. 4 summed) */
+    float depth;        /* common depth Z */
+    float depth_var;    /* its variance; SNR = depth / sqrt(depth_var) */
+    float t0;           /* t0_start + i_t0 * t0_stride, days */
+    int32_t i_t0;       /* cell of the first epoch, in [0, ceil(P/stride)) */
+    int32_t j_dur;      /* duration index */
+    int32_t n_transits; /* epochs that contributed (non-null cells) */
+    int32_t reserved;
+} cetra_peak;
+
+const char *cetra_status_string(int status);
+
+/* Number of SMs / shared memory the library will size its persistent grids for (device of the
+ * current context).  Returns CETRA_OK or CETRA_ERR_CUDA. */
+int cetra_device_info(int32_t *n_sm, int32_t *smem_per_block_optin);
+
+/* ------------------------------------------------------------------------------------------
+ * Linear search (§2.2).
+ *
+ *  times_host     [n]            float64 days, regular cadence
+ *  flux_dev       [n_lc][n]      dtype (float32 or float64), baseline 1
+ *  flux_err_dev   [n_lc][n]      dtype
+ *  durations_host [n_dur]        float64 days, > 0, n_dur <= CETRA_MAX_DURATIONS
+ *  template_host  [n_template]   float32, tpl[0] = first contact ... tpl[n_template-1] = last contact,
+ *                                normalised to maximum depth 1; sampled nearest-
+ *                                neighbour: idx = floor(x*(M-1)+1/2), x = (t_n - t_i)/D_j + 1/2 (R3)
+ *  depth_dev, var_dev, dlogL_dev  [n_lc][n_dur][n_t0] float32 outputs (any of them may be NULL):
+ *        depth = S_wmf/S_wmm,  var = 1/S_wmm,  dlogL = Eq. 2 = 1/2 S_wmf^2/S_wmm.
+ *  stats_dev      optional output (may be NULL): the sufficient statistics (S_wmm, S_wmf) as float2,
+ *                 [n_lc][n_dur][cetra_stats_pitch(n_t0)], zero in null cells and in the row padding;
+ *                 this is the form cetra_periodic_search_stats consumes.
+ * ------------------------------------------------------------------------------------------ */
+size_t cetra_linear_workspace_bytes(const double *times_host, int64_t n, int32_t n_lc,
+                                    const double *durations_host, int32_t n_dur,
+                                    cetra_t0_grid grid, int32_t n_template);
+
+int cetra_linear_search(const double *times_host, const void *flux_dev, const void *flux_err_dev,
+                        cetra_dtype dtype, int64_t n, int32_t n_lc,
+                        const double *durations_host, int32_t n_dur, cetra_t0_grid grid,
+                        const float *template_host, int32_t n_template,
+                        float *depth_dev, float *var_dev, float *dlogL_dev, float *stats_dev,
+                        void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* Row pitch (in cells) of the sufficient-statistics grid for n_t0 cells. */
+int64_t cetra_stats_pitch(int64_t n_t0);
+
+/* ------------------------------------------------------------------------------------------
+ * Periodic search (§2.3).
+ *
+ *  depth_dev, var_dev, dlogL_dev  [n_lc][n_dur][n_t0] float32: the linear-search grids.  (dlogL is
+ *        accepted for symmetry with the paper's interface; Eq. 4 summed at the common depth depends
+ *        on it only through 1/2 depth^2/var.)
+ *  periods_host   [n_per] float64 days, each >= t0_stride
+ *  dur_lo_host, dur_hi_host  optional [n_per] int32: half-open duration-index range searched for each
+ *        period; NULL = every duration.  Durations with D_j >= P_k are always skipped
+ *        (PAPER.md:145).
+ *  peaks_dev      [n_lc][n_per] output records.  Ties in lr: smallest j_dur, then smallest i_t0 (R13).
+ *
+ * Epoch e of phase p uses cell p + llrint(e * (P/stride)) (FP64, R11) while that is <= n_t0-1.
+ * ------------------------------------------------------------------------------------------ */
+size_t cetra_periodic_workspace_bytes(int32_t n_lc, int32_t n_dur, cetra_t0_grid grid, int32_t n_per);
+
+int cetra_periodic_search(const float *depth_dev, const float *var_dev, const float *dlogL_dev,
+                          int32_t n_lc, int32_t n_dur, cetra_t0_grid grid,
+                          const double *durations_host, const double *periods_host, int32_t n_per,
+                          const int32_t *dur_lo_host, const int32_t *dur_hi_host,
+                          cetra_peak *peaks_dev,
+                          void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* Same search on the sufficient statistics written by cetra_linear_search (stats_dev). */
+int cetra_periodic_search_stats(const float *stats_dev, int32_t n_lc, int32_t n_dur, cetra_t0_grid grid,
+                                const double *durations_host, const double *periods_host, int32_t n_per,
+                                const int32_t *dur_lo_host, const int32_t *dur_hi_host,
+                                cetra_peak *peaks_dev,
+                                void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* ------------------------------------------------------------------------------------------
+ * Batched search: n_lc light curves sharing one timestamp array, linear search then
+ * periodic search per chunk of light curves; the per-curve grids live only in the workspace.
+ * Arguments as above.  `lc_chunk` light curves are resident at a time (0 = library default).
+ * ------------------------------------------------------------------------------------------ */
+size_t cetra_search_batched_workspace_bytes(const double *times_host, int64_t n, int32_t n_lc, int32_t lc_chunk,
+                                            const double *durations_host, int32_t n_dur, cetra_t0_grid grid,
+                                            int32_t n_template, int32_t n_per);
+
+int cetra_search_batched(const double *times_host, const void *flux_dev, const void *flux_err_dev,
+                         cetra_dtype dtype, int64_t n, int32_t n_lc, int32_t lc_chunk,
+                         const double *durations_host, int32_t n_dur, cetra_t0_grid grid,
+                         const float *template_host, int32_t n_template,
+                         const double *periods_host, int32_t n_per,
+                         const int32_t *dur_lo_host, const int32_t *dur_hi_host,
+                         cetra_peak *peaks_dev,
+                         void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* Same, with the light curves and the result in HOST memory (pinned memory recommended): each chunk is
+ * copied host->device, searched, and its records copied device->host on `cuda_stream`; the call
+ * synchronises the stream before returning.  The workspace must be
+ * cetra_search_batched_host_workspace_bytes (it also stages the inputs and the records). */
+size_t cetra_search_batched_host_workspace_bytes(const double *times_host, int64_t n, int32_t n_lc, int32_t lc_chunk,
+                                                 cetra_dtype dtype,
+                                                 const double *durations_host, int32_t n_dur, cetra_t0_grid grid,
+                                                 int32_t n_template, int32_t n_per);
+
+int cetra_search_batched_host(const double *times_host, const void *flux_host, const void *flux_err_host,
+                              cetra_dtype dtype, int64_t n, int32_t n_lc, int32_t lc_chunk,
+                              const double *durations_host, int32_t n_dur, cetra_t0_grid grid,
+                              const float *template_host, int32_t n_template,
+                              const double *periods_host, int32_t n_per,
+                              const int32_t *dur_lo_host, const int32_t *dur_hi_host,
+                              cetra_peak *peaks_host,
+                              void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* Number of kernel launches the library has enqueued since the process started (diagnostic). */
+int64_t cetra_kernel_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CETRA_H_ */

@@ -1,0 +1,402 @@
+"""ctypes binding of libcetra_b200.so (include/cetra.h) -- argument marshalling only.
+
+Every function has the name of the C entry point it calls.  Device arrays are torch CUDA tensors
+(PyTorch is used for device memory and streams only); small grids are numpy/host arrays.  All the
+arithmetic of the path runs in the CUDA kernels; there is no CPU fallback: if the library cannot be
+loaded, or no CUDA device is present, the compute calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+from typing import Optional, Sequence
+
+import numpy as np
+
+from . import build as _build
+
+CETRA_OK = 0
+CETRA_ERR_INVALID_ARG = -1
+CETRA_ERR_NONUNIFORM_TIMES = -2
+CETRA_ERR_UNSUPPORTED = -3
+CETRA_ERR_WORKSPACE = -4
+CETRA_ERR_CUDA = -5
+CETRA_F32, CETRA_F64 = 0, 1
+CETRA_MAX_DURATIONS = 128
+
+# Every symbol include/cetra.h declares (tests check that the library exports each of them).
+EXPORTED_SYMBOLS = (
+    "cetra_status_string", "cetra_device_info", "cetra_stats_pitch", "cetra_kernel_launch_count",
+    "cetra_linear_workspace_bytes", "cetra_linear_search",
+    "cetra_periodic_workspace_bytes", "cetra_periodic_search", "cetra_periodic_search_stats",
+    "cetra_search_batched_workspace_bytes", "cetra_search_batched",
+    "cetra_search_batched_host_workspace_bytes", "cetra_search_batched_host",
+)
+
+
+class CetraError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {status_string(status)} (status {status})")
+
+
+class cetra_t0_grid(ctypes.Structure):
+    _fields_ = [("t0_start", ctypes.c_double), ("t0_stride", ctypes.c_double), ("n_t0", ctypes.c_int64)]
+
+
+class cetra_peak(ctypes.Structure):
+    _fields_ = [("lr", ctypes.c_float), ("depth", ctypes.c_float), ("depth_var", ctypes.c_float),
+                ("t0", ctypes.c_float), ("i_t0", ctypes.c_int32), ("j_dur", ctypes.c_int32),
+                ("n_transits", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+
+
+PEAK_DTYPE = np.dtype([("lr", "<f4"), ("depth", "<f4"), ("depth_var", "<f4"), ("t0", "<f4"),
+                       ("i_t0", "<i4"), ("j_dur", "<i4"), ("n_transits", "<i4"), ("reserved", "<i4")])
+assert PEAK_DTYPE.itemsize == ctypes.sizeof(cetra_peak) == 32
+
+_lib: Optional[ctypes.CDLL] = None
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen the in-tree library (building it with nvcc first if it is missing or stale)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB_PATH
+    if not os.path.exists(path) or os.environ.get("CETRA_REBUILD") == "1":
+        path = _build.build()
+    lib = ctypes.CDLL(path)
+    vp, dp, fp, ip = ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.c_void_p, ctypes.c_void_p
+    i32, i64, sz = ctypes.c_int32, ctypes.c_int64, ctypes.c_size_t
+    lib.cetra_status_string.restype = ctypes.c_char_p
+    lib.cetra_status_string.argtypes = [ctypes.c_int]
+    lib.cetra_device_info.restype = ctypes.c_int
+    lib.cetra_device_info.argtypes = [ctypes.POINTER(i32), ctypes.POINTER(i32)]
+    lib.cetra_stats_pitch.restype = i64
+    lib.cetra_stats_pitch.argtypes = [i64]
+    lib.cetra_kernel_launch_count.restype = i64
+    lib.cetra_kernel_launch_count.argtypes = []
+    lib.cetra_linear_workspace_bytes.restype = sz
+    lib.cetra_linear_workspace_bytes.argtypes = [dp, i64, i32, dp, i32, cetra_t0_grid, i32]
+    lib.cetra_linear_search.restype = ctypes.c_int
+    lib.cetra_linear_search.argtypes = [dp, vp, vp, ctypes.c_int, i64, i32, dp, i32, cetra_t0_grid, fp, i32,
+                                        vp, vp, vp, vp, vp, sz, vp]
+    lib.cetra_periodic_workspace_bytes.restype = sz
+    lib.cetra_periodic_workspace_bytes.argtypes = [i32, i32, cetra_t0_grid, i32]
+    lib.cetra_periodic_search.restype = ctypes.c_int
+    lib.cetra_periodic_search.argtypes = [vp, vp, vp, i32, i32, cetra_t0_grid, dp, dp, i32, ip, ip, vp, vp, sz, vp]
+    lib.cetra_periodic_search_stats.restype = ctypes.c_int
+    lib.cetra_periodic_search_stats.argtypes = [vp, i32, i32, cetra_t0_grid, dp, dp, i32, ip, ip, vp, vp, sz, vp]
+    lib.cetra_search_batched_workspace_bytes.restype = sz
+    lib.cetra_search_batched_workspace_bytes.argtypes = [dp, i64, i32, i32, dp, i32, cetra_t0_grid, i32, i32]
+    lib.cetra_search_batched.restype = ctypes.c_int
+    lib.cetra_search_batched.argtypes = [dp, vp, vp, ctypes.c_int, i64, i32, i32, dp, i32, cetra_t0_grid, fp, i32,
+                                         dp, i32, ip, ip, vp, vp, sz, vp]
+    lib.cetra_search_batched_host_workspace_bytes.restype = sz
+    lib.cetra_search_batched_host_workspace_bytes.argtypes = [dp, i64, i32, i32, ctypes.c_int, dp, i32,
+                                                              cetra_t0_grid, i32, i32]
+    lib.cetra_search_batched_host.restype = ctypes.c_int
+    lib.cetra_search_batched_host.argtypes = [dp, vp, vp, ctypes.c_int, i64, i32, i32, dp, i32, cetra_t0_grid, fp,
+                                              i32, dp, i32, ip, ip, vp, vp, sz, vp]
+    _lib = lib
+    return lib
+
+
+def status_string(status: int) -> str:
+    return load_library().cetra_status_string(int(status)).decode()
+
+
+def _check(status: int, where: str) -> None:
+    if status != CETRA_OK:
+        raise CetraError(status, where)
+
+
+def _f64(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _dp(a: np.ndarray):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _opt_i32(a):
+    if a is None:
+        return None, None
+    arr = np.ascontiguousarray(a, dtype=np.int32)
+    return arr, arr.ctypes.data
+
+
+def _grid(t0_start: float, t0_stride: float, n_t0: int) -> cetra_t0_grid:
+    return cetra_t0_grid(float(t0_start), float(t0_stride), int(n_t0))
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2503_20875_b200 needs a CUDA device: there is no CPU fallback")
+    return torch
+
+
+def _stream_ptr(torch, stream) -> int:
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return int(s.cuda_stream)
+
+
+def _dtype_code(torch, t) -> int:
+    if t.dtype == torch.float32:
+        return CETRA_F32
+    if t.dtype == torch.float64:
+        return CETRA_F64
+    raise TypeError(f"flux must be float32 or float64, got {t.dtype}")
+
+
+def _dev_input(torch, flux, flux_err):
+    if not (flux.is_cuda and flux_err.is_cuda):
+        raise TypeError("flux and flux_err must be CUDA tensors")
+    if flux.dtype != flux_err.dtype or flux.shape != flux_err.shape:
+        raise TypeError("flux and flux_err must have the same dtype and shape")
+    flux, flux_err = flux.contiguous(), flux_err.contiguous()
+    if flux.dim() == 1:
+        n_lc, n = 1, flux.shape[0]
+    elif flux.dim() == 2:
+        n_lc, n = flux.shape
+    else:
+        raise TypeError("flux must be [N] or [B][N]")
+    return flux, flux_err, int(n_lc), int(n)
+
+
+def _workspace(torch, nbytes: int, device, workspace=None):
+    if workspace is not None:
+        if workspace.dtype != torch.uint8 or not workspace.is_cuda or workspace.numel() < nbytes:
+            raise CetraError(CETRA_ERR_WORKSPACE, "workspace")
+        return workspace
+    return torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
+
+
+def cetra_device_info():
+    lib = load_library()
+    a, b = ctypes.c_int32(), ctypes.c_int32()
+    _check(lib.cetra_device_info(ctypes.byref(a), ctypes.byref(b)), "cetra_device_info")
+    return a.value, b.value
+
+
+def cetra_stats_pitch(n_t0: int) -> int:
+    return int(load_library().cetra_stats_pitch(int(n_t0)))
+
+
+def cetra_kernel_launch_count() -> int:
+    return int(load_library().cetra_kernel_launch_count())
+
+
+def cetra_linear_workspace_bytes(times, n_lc: int, durations, t0_start, t0_stride, n_t0, n_template: int) -> int:
+    lib = load_library()
+    times, durations = _f64(times), _f64(durations)
+    return int(lib.cetra_linear_workspace_bytes(_dp(times), times.shape[0], int(n_lc), _dp(durations),
+                                                durations.shape[0], _grid(t0_start, t0_stride, n_t0),
+                                                int(n_template)))
+
+
+@dataclass
+class LinearResult:
+    """Outputs of cetra_linear_search: float32 CUDA tensors [B][J][I] (or [J][I] for a 1-D input)."""
+    depth: object
+    depth_var: object
+    dlogL: object
+    stats: object          # [B][J][pitch][2] (S_wmm, S_wmf) or None
+
+
+def cetra_linear_search(times, flux, flux_err, durations, t0_start: float, t0_stride: float, n_t0: int, template,
+                        want_grids: bool = True, want_stats: bool = False, workspace=None,
+                        stream=None) -> LinearResult:
+    torch = _torch()
+    lib = load_library()
+    flux, flux_err, n_lc, n = _dev_input(torch, flux, flux_err)
+    squeeze = flux.dim() == 1
+    times, durations = _f64(times), _f64(durations)
+    tpl = np.ascontiguousarray(template, dtype=np.float32)
+    if times.shape[0] != n:
+        raise CetraError(CETRA_ERR_INVALID_ARG, "cetra_linear_search: len(times) != flux.shape[-1]")
+    grid = _grid(t0_start, t0_stride, n_t0)
+    n_dur = durations.shape[0]
+    nbytes = int(lib.cetra_linear_workspace_bytes(_dp(times), n, n_lc, _dp(durations), n_dur, grid, tpl.shape[0]))
+    if nbytes == 0:
+        # let the entry point report the precise status
+        nbytes = 256
+    ws = _workspace(torch, nbytes, flux.device, workspace)
+    dev = flux.device
+    depth = var = dl = stats = None
+    if want_grids:
+        depth = torch.empty((n_lc, n_dur, n_t0), dtype=torch.float32, device=dev)
+        var = torch.empty_like(depth)
+        dl = torch.empty_like(depth)
+    if want_stats:
+        stats = torch.empty((n_lc, n_dur, cetra_stats_pitch(n_t0), 2), dtype=torch.float32, device=dev)
+    ptr = lambda t: t.data_ptr() if t is not None else None
+    with torch.cuda.device(dev):
+        rc = lib.cetra_linear_search(_dp(times), flux.data_ptr(), flux_err.data_ptr(), _dtype_code(torch, flux), n,
+                                     n_lc, _dp(durations), n_dur, grid, tpl.ctypes.data, tpl.shape[0], ptr(depth),
+                                     ptr(var), ptr(dl), ptr(stats), ws.data_ptr(), ws.numel(),
+                                     _stream_ptr(torch, stream))
+    _check(rc, "cetra_linear_search")
+    if squeeze and want_grids:
+        depth, var, dl = depth[0], var[0], dl[0]
+    return LinearResult(depth, var, dl, stats)
+
+
+def cetra_periodic_workspace_bytes(n_lc: int, n_dur: int, t0_start, t0_stride, n_t0, n_per: int) -> int:
+    return int(load_library().cetra_periodic_workspace_bytes(int(n_lc), int(n_dur), _grid(t0_start, t0_stride, n_t0),
+                                                             int(n_per)))
+
+
+def _peaks_tensor(torch, n_lc: int, n_per: int, device):
+    return torch.empty((n_lc, n_per, 8), dtype=torch.int32, device=device)
+
+
+def peaks_to_numpy(peaks) -> np.ndarray:
+    """[B][K][8] int32 tensor of cetra_peak records -> numpy structured array [B][K] (PEAK_DTYPE)."""
+    arr = peaks.detach().cpu().numpy()
+    return np.ascontiguousarray(arr).view(PEAK_DTYPE).reshape(arr.shape[:-1])
+
+
+def cetra_periodic_search(depth, depth_var, dlogL, t0_start: float, t0_stride: float, durations, periods,
+                          dur_lo=None, dur_hi=None, workspace=None, stream=None):
+    """Returns a CUDA int32 tensor [B][K][8] holding cetra_peak records (see peaks_to_numpy)."""
+    torch = _torch()
+    lib = load_library()
+    for t in (depth, depth_var, dlogL):
+        if not t.is_cuda or t.dtype != torch.float32:
+            raise TypeError("linear-search grids must be float32 CUDA tensors")
+    depth, depth_var, dlogL = depth.contiguous(), depth_var.contiguous(), dlogL.contiguous()
+    if depth.dim() == 2:
+        n_lc, (n_dur, n_t0) = 1, depth.shape
+    else:
+        n_lc, n_dur, n_t0 = depth.shape
+    durations, periods = _f64(durations), _f64(periods)
+    lo_arr, lo = _opt_i32(dur_lo)
+    hi_arr, hi = _opt_i32(dur_hi)
+    grid = _grid(t0_start, t0_stride, n_t0)
+    n_per = periods.shape[0]
+    nbytes = int(lib.cetra_periodic_workspace_bytes(n_lc, n_dur, grid, n_per))
+    ws = _workspace(torch, nbytes, depth.device, workspace)
+    peaks = _peaks_tensor(torch, n_lc, n_per, depth.device)
+    with torch.cuda.device(depth.device):
+        rc = lib.cetra_periodic_search(depth.data_ptr(), depth_var.data_ptr(), dlogL.data_ptr(), n_lc, n_dur, grid,
+                                       _dp(durations), _dp(periods), n_per, lo, hi, peaks.data_ptr(), ws.data_ptr(),
+                                       ws.numel(), _stream_ptr(torch, stream))
+    _check(rc, "cetra_periodic_search")
+    return peaks
+
+
+def cetra_periodic_search_stats(stats, n_t0: int, t0_start: float, t0_stride: float, durations, periods,
+                                dur_lo=None, dur_hi=None, workspace=None, stream=None):
+    torch = _torch()
+    lib = load_library()
+    if not stats.is_cuda or stats.dtype != torch.float32 or stats.dim() != 4 or stats.shape[-1] != 2:
+        raise TypeError("stats must be a float32 CUDA tensor [B][J][pitch][2]")
+    stats = stats.contiguous()
+    n_lc, n_dur, pitch, _ = stats.shape
+    if pitch != cetra_stats_pitch(n_t0):
+        raise CetraError(CETRA_ERR_INVALID_ARG, "cetra_periodic_search_stats: wrong row pitch")
+    durations, periods = _f64(durations), _f64(periods)
+    lo_arr, lo = _opt_i32(dur_lo)
+    hi_arr, hi = _opt_i32(dur_hi)
+    grid = _grid(t0_start, t0_stride, n_t0)
+    n_per = periods.shape[0]
+    nbytes = int(lib.cetra_periodic_workspace_bytes(n_lc, n_dur, grid, n_per))
+    ws = _workspace(torch, nbytes, stats.device, workspace)
+    peaks = _peaks_tensor(torch, n_lc, n_per, stats.device)
+    with torch.cuda.device(stats.device):
+        rc = lib.cetra_periodic_search_stats(stats.data_ptr(), n_lc, n_dur, grid, _dp(durations), _dp(periods), n_per,
+                                             lo, hi, peaks.data_ptr(), ws.data_ptr(), ws.numel(),
+                                             _stream_ptr(torch, stream))
+    _check(rc, "cetra_periodic_search_stats")
+    return peaks
+
+
+def cetra_search_batched_workspace_bytes(times, n_lc: int, lc_chunk: int, durations, t0_start, t0_stride, n_t0,
+                                         n_template: int, n_per: int) -> int:
+    lib = load_library()
+    times, durations = _f64(times), _f64(durations)
+    return int(lib.cetra_search_batched_workspace_bytes(_dp(times), times.shape[0], int(n_lc), int(lc_chunk),
+                                                        _dp(durations), durations.shape[0],
+                                                        _grid(t0_start, t0_stride, n_t0), int(n_template), int(n_per)))
+
+
+def cetra_search_batched(times, flux, flux_err, durations, t0_start: float, t0_stride: float, n_t0: int, template,
+                         periods, dur_lo=None, dur_hi=None, lc_chunk: int = 0, workspace=None, peaks=None,
+                         stream=None):
+    """Linear + periodic search of [B][N] device light curves sharing `times`; returns peaks [B][K][8] int32."""
+    torch = _torch()
+    lib = load_library()
+    flux, flux_err, n_lc, n = _dev_input(torch, flux, flux_err)
+    times, durations, periods = _f64(times), _f64(durations), _f64(periods)
+    tpl = np.ascontiguousarray(template, dtype=np.float32)
+    if times.shape[0] != n:
+        raise CetraError(CETRA_ERR_INVALID_ARG, "cetra_search_batched: len(times) != flux.shape[-1]")
+    lo_arr, lo = _opt_i32(dur_lo)
+    hi_arr, hi = _opt_i32(dur_hi)
+    grid = _grid(t0_start, t0_stride, n_t0)
+    n_dur, n_per = durations.shape[0], periods.shape[0]
+    nbytes = int(lib.cetra_search_batched_workspace_bytes(_dp(times), n, n_lc, int(lc_chunk), _dp(durations), n_dur,
+                                                          grid, tpl.shape[0], n_per))
+    ws = _workspace(torch, nbytes, flux.device, workspace)
+    if peaks is None:
+        peaks = _peaks_tensor(torch, n_lc, n_per, flux.device)
+    with torch.cuda.device(flux.device):
+        rc = lib.cetra_search_batched(_dp(times), flux.data_ptr(), flux_err.data_ptr(), _dtype_code(torch, flux), n,
+                                      n_lc, int(lc_chunk), _dp(durations), n_dur, grid, tpl.ctypes.data, tpl.shape[0],
+                                      _dp(periods), n_per, lo, hi, peaks.data_ptr(), ws.data_ptr(), ws.numel(),
+                                      _stream_ptr(torch, stream))
+    _check(rc, "cetra_search_batched")
+    return peaks
+
+
+def cetra_search_batched_host_workspace_bytes(times, n_lc: int, lc_chunk: int, dtype_code: int, durations, t0_start,
+                                              t0_stride, n_t0, n_template: int, n_per: int) -> int:
+    lib = load_library()
+    times, durations = _f64(times), _f64(durations)
+    return int(lib.cetra_search_batched_host_workspace_bytes(_dp(times), times.shape[0], int(n_lc), int(lc_chunk),
+                                                             int(dtype_code), _dp(durations), durations.shape[0],
+                                                             _grid(t0_start, t0_stride, n_t0), int(n_template),
+                                                             int(n_per)))
+
+
+def cetra_search_batched_host(times, flux_host, flux_err_host, durations, t0_start: float, t0_stride: float,
+                              n_t0: int, template, periods, dur_lo=None, dur_hi=None, lc_chunk: int = 0,
+                              workspace=None, peaks_host=None, device=None, stream=None) -> np.ndarray:
+    """Same search with HOST light curves (torch CPU tensors, ideally pinned, or numpy arrays) and a HOST
+    result: the library copies each chunk in, searches it and copies the records out.  Returns a numpy
+    structured array [B][K] of PEAK_DTYPE viewing `peaks_host`."""
+    torch = _torch()
+    lib = load_library()
+    if isinstance(flux_host, np.ndarray):
+        flux_host, flux_err_host = torch.from_numpy(flux_host), torch.from_numpy(flux_err_host)
+    if flux_host.is_cuda or flux_err_host.is_cuda:
+        raise TypeError("cetra_search_batched_host takes host tensors")
+    flux_host, flux_err_host = flux_host.contiguous(), flux_err_host.contiguous()
+    if flux_host.dtype != flux_err_host.dtype or flux_host.shape != flux_err_host.shape or flux_host.dim() != 2:
+        raise TypeError("flux and flux_err must be [B][N] host tensors of one dtype")
+    n_lc, n = (int(x) for x in flux_host.shape)
+    times, durations, periods = _f64(times), _f64(durations), _f64(periods)
+    tpl = np.ascontiguousarray(template, dtype=np.float32)
+    if times.shape[0] != n:
+        raise CetraError(CETRA_ERR_INVALID_ARG, "cetra_search_batched_host: len(times) != flux.shape[-1]")
+    lo_arr, lo = _opt_i32(dur_lo)
+    hi_arr, hi = _opt_i32(dur_hi)
+    grid = _grid(t0_start, t0_stride, n_t0)
+    n_dur, n_per = durations.shape[0], periods.shape[0]
+    code = _dtype_code(torch, flux_host)
+    dev = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+    nbytes = int(lib.cetra_search_batched_host_workspace_bytes(_dp(times), n, n_lc, int(lc_chunk), code,
+                                                               _dp(durations), n_dur, grid, tpl.shape[0], n_per))
+    ws = _workspace(torch, nbytes, dev, workspace)
+    if peaks_host is None:
+        peaks_host = torch.empty((n_lc, n_per, 8), dtype=torch.int32, pin_memory=True)
+    with torch.cuda.device(dev):
+        rc = lib.cetra_search_batched_host(_dp(times), flux_host.data_ptr(), flux_err_host.data_ptr(), code, n, n_lc,
+                                           int(lc_chunk), _dp(durations), n_dur, grid, tpl.ctypes.data, tpl.shape[0],
+                                           _dp(periods), n_per, lo, hi, peaks_host.data_ptr(), ws.data_ptr(),
+                                           ws.numel(), _stream_ptr(torch, stream))
+    _check(rc, "cetra_search_batched_host")
+    return peaks_host.numpy().view(PEAK_DTYPE).reshape(n_lc, n_per)

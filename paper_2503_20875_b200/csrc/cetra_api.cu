@@ -1,0 +1,343 @@
+// C ABI of the CETRA B200 library: argument validation, workspace carve-up, launch order.
+// Every step of the path runs in the kernels of linear_search.cu / periodic_search.cu; nothing here
+// computes any of the method's arithmetic on the host, and there is no CPU fallback.
+#include <math.h>
+#include <string.h>
+
+#include <algorithm>
+
+#include "linear_search.cuh"
+#include "periodic_search.cuh"
+
+namespace cetra {
+
+std::atomic<int64_t> g_launch_count{0};
+
+// DESIGN.md R1/R9: the samples are a regular grid; the t0 grid sits on it with a whole-sample stride.
+int derive_geometry(const double *times_host, int64_t n, cetra_t0_grid grid, Geometry *g) {
+    if (!times_host || n < 2 || !(grid.t0_stride > 0.0) || !std::isfinite(grid.t0_stride) ||
+        !std::isfinite(grid.t0_start) || grid.n_t0 < 1)
+        return CETRA_ERR_INVALID_ARG;
+    const double c = (times_host[n - 1] - times_host[0]) / static_cast<double>(n - 1);
+    if (!(c > 0.0) || !std::isfinite(c)) return CETRA_ERR_INVALID_ARG;
+    for (int64_t i = 0; i < n; ++i)
+        if (!(fabs(times_host[i] - times_host[0] - static_cast<double>(i) * c) <= 1e-3 * c))
+            return CETRA_ERR_NONUNIFORM_TIMES;
+    const double a = (grid.t0_start - times_host[0]) / c;
+    const double b = grid.t0_stride / c;
+    if (!(fabs(a) < 1e15) || !(b < 1e15)) return CETRA_ERR_UNSUPPORTED;
+    const long long ia = llrint(a), ib = llrint(b);
+    if (fabs(a - static_cast<double>(ia)) > 1e-6 || fabs(b - static_cast<double>(ib)) > 1e-6 || ib < 1)
+        return CETRA_ERR_UNSUPPORTED;
+    g->cadence = c;
+    g->n0 = ia;
+    g->q = ib;
+    return CETRA_OK;
+}
+
+struct Device {
+    int n_sm = 0, smem_optin = 0;
+};
+
+static int query_device(Device *d) {
+    int dev = 0;
+    CETRA_CUDA_TRY(cudaGetDevice(&dev));
+    CETRA_CUDA_TRY(cudaDeviceGetAttribute(&d->n_sm, cudaDevAttrMultiProcessorCount, dev));
+    CETRA_CUDA_TRY(cudaDeviceGetAttribute(&d->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    return CETRA_OK;
+}
+
+// Plans are sized for a B200 when no device is visible (workspace queries on a CPU-only host).
+static Device device_or_default() {
+    Device d;
+    if (query_device(&d) != CETRA_OK || d.n_sm <= 0) {
+        cudaGetLastError();
+        d.n_sm = 148;
+        d.smem_optin = 232448;
+    }
+    return d;
+}
+
+// The compute entry points refuse to run without a device: there is no CPU fallback.
+static int require_device() {
+    Device d;
+    const int rc = query_device(&d);
+    if (rc != CETRA_OK) cudaGetLastError();
+    return rc;
+}
+
+static bool aligned(const void *p) { return (reinterpret_cast<uintptr_t>(p) & (kAlign - 1)) == 0; }
+
+static size_t stats_bytes(int32_t n_lc, int32_t n_dur, int64_t n_t0) {
+    return align_up(sizeof(float2) * static_cast<size_t>(n_lc) * n_dur * static_cast<size_t>(cetra_stats_pitch(n_t0)));
+}
+
+static size_t dtype_size(cetra_dtype t) { return t == CETRA_F64 ? 8 : 4; }
+
+}  // namespace cetra
+
+using namespace cetra;
+
+extern "C" {
+
+const char *cetra_status_string(int status) {
+    switch (status) {
+        case CETRA_OK: return "ok";
+        case CETRA_ERR_INVALID_ARG: return "invalid argument";
+        case CETRA_ERR_NONUNIFORM_TIMES: return "times[] is not a regular grid";
+        case CETRA_ERR_UNSUPPORTED: return "unsupported configuration";
+        case CETRA_ERR_WORKSPACE: return "workspace null, misaligned or too small";
+        case CETRA_ERR_CUDA: return "CUDA runtime error";
+        default: return "unknown status";
+    }
+}
+
+int cetra_device_info(int32_t *n_sm, int32_t *smem_per_block_optin) {
+    Device d;
+    const int rc = query_device(&d);
+    if (rc != CETRA_OK) return rc;
+    if (n_sm) *n_sm = d.n_sm;
+    if (smem_per_block_optin) *smem_per_block_optin = d.smem_optin;
+    return CETRA_OK;
+}
+
+int64_t cetra_stats_pitch(int64_t n_t0) { return round_up64(n_t0 + kStatsPad, 32); }
+
+int64_t cetra_kernel_launch_count(void) { return g_launch_count.load(); }
+
+// ------------------------------------------------------------------------------------------ linear
+size_t cetra_linear_workspace_bytes(const double *times_host, int64_t n, int32_t n_lc, const double *durations_host,
+                                    int32_t n_dur, cetra_t0_grid grid, int32_t n_template) {
+    const Device d = device_or_default();
+    LinearPlan pl;
+    if (build_linear_plan(times_host, n, n_lc, durations_host, n_dur, grid, n_template, d.smem_optin, d.n_sm, &pl) !=
+        CETRA_OK)
+        return 0;
+    return linear_workspace_bytes(pl, n_lc, n_template);
+}
+
+int cetra_linear_search(const double *times_host, const void *flux_dev, const void *flux_err_dev, cetra_dtype dtype,
+                        int64_t n, int32_t n_lc, const double *durations_host, int32_t n_dur, cetra_t0_grid grid,
+                        const float *template_host, int32_t n_template, float *depth_dev, float *var_dev,
+                        float *dlogL_dev, float *stats_dev, void *workspace_dev, size_t workspace_bytes,
+                        void *cuda_stream) {
+    if (!flux_dev || !flux_err_dev || !template_host || (dtype != CETRA_F32 && dtype != CETRA_F64))
+        return CETRA_ERR_INVALID_ARG;
+    const Device d = device_or_default();   // argument errors are reported even where no device is visible
+    int rc;
+    LinearPlan pl;
+    rc = build_linear_plan(times_host, n, n_lc, durations_host, n_dur, grid, n_template, d.smem_optin, d.n_sm, &pl);
+    if (rc != CETRA_OK) return rc;
+    if (!workspace_dev || !aligned(workspace_dev) || workspace_bytes < linear_workspace_bytes(pl, n_lc, n_template))
+        return CETRA_ERR_WORKSPACE;
+    if ((rc = require_device()) != CETRA_OK) return rc;
+    return run_linear(pl, flux_dev, flux_err_dev, dtype, n, n_lc, template_host, n_template, false, depth_dev,
+                      var_dev, dlogL_dev, stats_dev, workspace_dev, static_cast<cudaStream_t>(cuda_stream));
+}
+
+// ---------------------------------------------------------------------------------------- periodic
+size_t cetra_periodic_workspace_bytes(int32_t n_lc, int32_t n_dur, cetra_t0_grid grid, int32_t n_per) {
+    if (n_lc < 1 || n_dur < 1 || n_per < 1 || grid.n_t0 < 1) return 0;
+    return periodic_workspace_bytes(n_lc, n_per) + stats_bytes(n_lc, n_dur, grid.n_t0);
+}
+
+int cetra_periodic_search_stats(const float *stats_dev, int32_t n_lc, int32_t n_dur, cetra_t0_grid grid,
+                                const double *durations_host, const double *periods_host, int32_t n_per,
+                                const int32_t *dur_lo_host, const int32_t *dur_hi_host, cetra_peak *peaks_dev,
+                                void *workspace_dev, size_t workspace_bytes, void *cuda_stream) {
+    if (!stats_dev || !peaks_dev || ((dur_lo_host == nullptr) != (dur_hi_host == nullptr)))
+        return CETRA_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(stats_dev) & 15) != 0) return CETRA_ERR_INVALID_ARG;
+    const Device d = device_or_default();   // argument errors are reported even where no device is visible
+    int rc;
+    PeriodicPlan pl;
+    rc = build_periodic_plan(n_lc, n_dur, grid, durations_host, periods_host, n_per, d.smem_optin, d.n_sm, &pl);
+    if (rc != CETRA_OK) return rc;
+    if (!workspace_dev || !aligned(workspace_dev) || workspace_bytes < periodic_workspace_bytes(n_lc, n_per))
+        return CETRA_ERR_WORKSPACE;
+    if ((rc = require_device()) != CETRA_OK) return rc;
+    return run_periodic(pl, reinterpret_cast<const float2 *>(stats_dev), periods_host, dur_lo_host, dur_hi_host, true,
+                        peaks_dev, workspace_dev, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int cetra_periodic_search(const float *depth_dev, const float *var_dev, const float *dlogL_dev, int32_t n_lc,
+                          int32_t n_dur, cetra_t0_grid grid, const double *durations_host,
+                          const double *periods_host, int32_t n_per, const int32_t *dur_lo_host,
+                          const int32_t *dur_hi_host, cetra_peak *peaks_dev, void *workspace_dev,
+                          size_t workspace_bytes, void *cuda_stream) {
+    (void)dlogL_dev;   // Eq. 4 summed at the common depth needs only depth and var (P4)
+    if (!depth_dev || !var_dev || !peaks_dev || ((dur_lo_host == nullptr) != (dur_hi_host == nullptr)))
+        return CETRA_ERR_INVALID_ARG;
+    const Device d = device_or_default();   // argument errors are reported even where no device is visible
+    int rc;
+    PeriodicPlan pl;
+    rc = build_periodic_plan(n_lc, n_dur, grid, durations_host, periods_host, n_per, d.smem_optin, d.n_sm, &pl);
+    if (rc != CETRA_OK) return rc;
+    if (!workspace_dev || !aligned(workspace_dev) ||
+        workspace_bytes < cetra_periodic_workspace_bytes(n_lc, n_dur, grid, n_per))
+        return CETRA_ERR_WORKSPACE;
+    if ((rc = require_device()) != CETRA_OK) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    char *ws = static_cast<char *>(workspace_dev);
+    float2 *stats = reinterpret_cast<float2 *>(ws + periodic_workspace_bytes(n_lc, n_per));
+    rc = run_grids_to_stats(depth_dev, var_dev, n_lc * n_dur, grid.n_t0, stats, st);
+    if (rc != CETRA_OK) return rc;
+    return run_periodic(pl, stats, periods_host, dur_lo_host, dur_hi_host, true, peaks_dev, workspace_dev, st);
+}
+
+// ----------------------------------------------------------------------------------------- batched
+namespace {
+
+struct BatchedLayout {
+    int32_t chunk = 0;
+    size_t linear_bytes = 0, stats_bytes = 0, periodic_bytes = 0, total = 0;
+};
+
+// Light curves resident at a time: by default as many as keep the chunk's (S_wmm, S_wmf) grids within
+// half of the 126 MB L2, so that the periodic search re-reads them from L2 and never from HBM.
+int32_t default_chunk(int32_t n_lc, int32_t n_dur, int64_t n_t0) {
+    const size_t per_lc = sizeof(float2) * static_cast<size_t>(n_dur) * static_cast<size_t>(cetra_stats_pitch(n_t0));
+    const size_t budget = 64ull << 20;
+    const size_t c = std::max<size_t>(1, budget / std::max<size_t>(per_lc, 1));
+    return static_cast<int32_t>(std::min<size_t>(c, static_cast<size_t>(n_lc)));
+}
+
+int plan_batched(const double *times_host, int64_t n, int32_t n_lc, int32_t lc_chunk, const double *durations_host,
+                 int32_t n_dur, cetra_t0_grid grid, int32_t n_template, int32_t n_per, const Device &d,
+                 LinearPlan *lin, BatchedLayout *lay) {
+    if (n_lc < 1 || lc_chunk < 0 || n_per < 1) return CETRA_ERR_INVALID_ARG;
+    if (n_dur < 1 || grid.n_t0 < 1) return CETRA_ERR_INVALID_ARG;
+    const int32_t chunk = lc_chunk > 0 ? std::min(lc_chunk, n_lc) : default_chunk(n_lc, n_dur, grid.n_t0);
+    const int rc = build_linear_plan(times_host, n, chunk, durations_host, n_dur, grid, n_template, d.smem_optin,
+                                     d.n_sm, lin);
+    if (rc != CETRA_OK) return rc;
+    lay->chunk = chunk;
+    lay->linear_bytes = linear_workspace_bytes(*lin, chunk, n_template);
+    lay->stats_bytes = stats_bytes(chunk, n_dur, grid.n_t0);
+    lay->periodic_bytes = periodic_workspace_bytes(chunk, n_per);
+    lay->total = lay->linear_bytes + lay->stats_bytes + lay->periodic_bytes;
+    return CETRA_OK;
+}
+
+// Linear search then periodic search for light curves [lc0, lc0 + m) of a chunked batch.
+int run_chunk(LinearPlan &lin, const BatchedLayout &lay, const Device &d, const void *flux_dev,
+              const void *flux_err_dev, cetra_dtype dtype, int64_t n, int32_t m, bool first,
+              const double *durations_host, int32_t n_dur, cetra_t0_grid grid, const float *template_host,
+              int32_t n_template, const double *periods_host, int32_t n_per, const int32_t *dur_lo_host,
+              const int32_t *dur_hi_host, cetra_peak *peaks_dev, char *ws, cudaStream_t st) {
+    float *stats = reinterpret_cast<float *>(ws + lay.linear_bytes);
+    int rc = run_linear(lin, flux_dev, flux_err_dev, dtype, n, m, template_host, n_template, false, nullptr, nullptr,
+                        nullptr, stats, ws, st);
+    if (rc != CETRA_OK) return rc;
+    PeriodicPlan per;
+    rc = build_periodic_plan(m, n_dur, grid, durations_host, periods_host, n_per, d.smem_optin, d.n_sm, &per);
+    if (rc != CETRA_OK) return rc;
+    return run_periodic(per, reinterpret_cast<const float2 *>(stats), periods_host, dur_lo_host, dur_hi_host, first,
+                        peaks_dev, ws + lay.linear_bytes + lay.stats_bytes, st);
+}
+
+}  // namespace
+
+size_t cetra_search_batched_workspace_bytes(const double *times_host, int64_t n, int32_t n_lc, int32_t lc_chunk,
+                                            const double *durations_host, int32_t n_dur, cetra_t0_grid grid,
+                                            int32_t n_template, int32_t n_per) {
+    const Device d = device_or_default();
+    LinearPlan lin;
+    BatchedLayout lay;
+    if (plan_batched(times_host, n, n_lc, lc_chunk, durations_host, n_dur, grid, n_template, n_per, d, &lin, &lay) !=
+        CETRA_OK)
+        return 0;
+    return lay.total;
+}
+
+int cetra_search_batched(const double *times_host, const void *flux_dev, const void *flux_err_dev, cetra_dtype dtype,
+                         int64_t n, int32_t n_lc, int32_t lc_chunk, const double *durations_host, int32_t n_dur,
+                         cetra_t0_grid grid, const float *template_host, int32_t n_template,
+                         const double *periods_host, int32_t n_per, const int32_t *dur_lo_host,
+                         const int32_t *dur_hi_host, cetra_peak *peaks_dev, void *workspace_dev,
+                         size_t workspace_bytes, void *cuda_stream) {
+    if (!flux_dev || !flux_err_dev || !template_host || !periods_host || !peaks_dev ||
+        (dtype != CETRA_F32 && dtype != CETRA_F64) || ((dur_lo_host == nullptr) != (dur_hi_host == nullptr)))
+        return CETRA_ERR_INVALID_ARG;
+    const Device d = device_or_default();   // argument errors are reported even where no device is visible
+    int rc;
+    LinearPlan lin;
+    BatchedLayout lay;
+    rc = plan_batched(times_host, n, n_lc, lc_chunk, durations_host, n_dur, grid, n_template, n_per, d, &lin, &lay);
+    if (rc != CETRA_OK) return rc;
+    if (!workspace_dev || !aligned(workspace_dev) || workspace_bytes < lay.total) return CETRA_ERR_WORKSPACE;
+    if ((rc = require_device()) != CETRA_OK) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const size_t esz = dtype_size(dtype);
+    for (int32_t lc0 = 0; lc0 < n_lc; lc0 += lay.chunk) {
+        const int32_t m = std::min(lay.chunk, n_lc - lc0);
+        const char *fl = static_cast<const char *>(flux_dev) + static_cast<size_t>(lc0) * n * esz;
+        const char *er = static_cast<const char *>(flux_err_dev) + static_cast<size_t>(lc0) * n * esz;
+        rc = run_chunk(lin, lay, d, fl, er, dtype, n, m, lc0 == 0, durations_host, n_dur, grid, template_host,
+                       n_template, periods_host, n_per, dur_lo_host, dur_hi_host,
+                       peaks_dev + static_cast<size_t>(lc0) * n_per, static_cast<char *>(workspace_dev), st);
+        if (rc != CETRA_OK) return rc;
+    }
+    return CETRA_OK;
+}
+
+size_t cetra_search_batched_host_workspace_bytes(const double *times_host, int64_t n, int32_t n_lc, int32_t lc_chunk,
+                                                 cetra_dtype dtype, const double *durations_host, int32_t n_dur,
+                                                 cetra_t0_grid grid, int32_t n_template, int32_t n_per) {
+    const Device d = device_or_default();
+    LinearPlan lin;
+    BatchedLayout lay;
+    if (plan_batched(times_host, n, n_lc, lc_chunk, durations_host, n_dur, grid, n_template, n_per, d, &lin, &lay) !=
+        CETRA_OK)
+        return 0;
+    const size_t in_bytes = align_up(static_cast<size_t>(lay.chunk) * n * dtype_size(dtype));
+    const size_t out_bytes = align_up(sizeof(cetra_peak) * static_cast<size_t>(lay.chunk) * n_per);
+    return lay.total + 2 * in_bytes + out_bytes;
+}
+
+int cetra_search_batched_host(const double *times_host, const void *flux_host, const void *flux_err_host,
+                              cetra_dtype dtype, int64_t n, int32_t n_lc, int32_t lc_chunk,
+                              const double *durations_host, int32_t n_dur, cetra_t0_grid grid,
+                              const float *template_host, int32_t n_template, const double *periods_host,
+                              int32_t n_per, const int32_t *dur_lo_host, const int32_t *dur_hi_host,
+                              cetra_peak *peaks_host, void *workspace_dev, size_t workspace_bytes,
+                              void *cuda_stream) {
+    if (!flux_host || !flux_err_host || !template_host || !periods_host || !peaks_host ||
+        (dtype != CETRA_F32 && dtype != CETRA_F64) || ((dur_lo_host == nullptr) != (dur_hi_host == nullptr)))
+        return CETRA_ERR_INVALID_ARG;
+    const Device d = device_or_default();   // argument errors are reported even where no device is visible
+    int rc;
+    LinearPlan lin;
+    BatchedLayout lay;
+    rc = plan_batched(times_host, n, n_lc, lc_chunk, durations_host, n_dur, grid, n_template, n_per, d, &lin, &lay);
+    if (rc != CETRA_OK) return rc;
+    const size_t esz = dtype_size(dtype);
+    const size_t in_bytes = align_up(static_cast<size_t>(lay.chunk) * n * esz);
+    const size_t out_bytes = align_up(sizeof(cetra_peak) * static_cast<size_t>(lay.chunk) * n_per);
+    if (!workspace_dev || !aligned(workspace_dev) || workspace_bytes < lay.total + 2 * in_bytes + out_bytes)
+        return CETRA_ERR_WORKSPACE;
+    if ((rc = require_device()) != CETRA_OK) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    char *ws = static_cast<char *>(workspace_dev);
+    char *fl_dev = ws + lay.total;
+    char *er_dev = fl_dev + in_bytes;
+    cetra_peak *pk_dev = reinterpret_cast<cetra_peak *>(er_dev + in_bytes);
+    for (int32_t lc0 = 0; lc0 < n_lc; lc0 += lay.chunk) {
+        const int32_t m = std::min(lay.chunk, n_lc - lc0);
+        const size_t bytes = static_cast<size_t>(m) * n * esz;
+        const char *fl = static_cast<const char *>(flux_host) + static_cast<size_t>(lc0) * n * esz;
+        const char *er = static_cast<const char *>(flux_err_host) + static_cast<size_t>(lc0) * n * esz;
+        CETRA_CUDA_TRY(cudaMemcpyAsync(fl_dev, fl, bytes, cudaMemcpyHostToDevice, st));
+        CETRA_CUDA_TRY(cudaMemcpyAsync(er_dev, er, bytes, cudaMemcpyHostToDevice, st));
+        rc = run_chunk(lin, lay, d, fl_dev, er_dev, dtype, n, m, lc0 == 0, durations_host, n_dur, grid,
+                       template_host, n_template, periods_host, n_per, dur_lo_host, dur_hi_host, pk_dev, ws, st);
+        if (rc != CETRA_OK) return rc;
+        CETRA_CUDA_TRY(cudaMemcpyAsync(peaks_host + static_cast<size_t>(lc0) * n_per, pk_dev,
+                                       sizeof(cetra_peak) * static_cast<size_t>(m) * n_per, cudaMemcpyDeviceToHost,
+                                       st));
+    }
+    CETRA_CUDA_TRY(cudaStreamSynchronize(st));
+    return CETRA_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,326 @@
+// Linear search (§2.2, lines 89-125): steps L0-L3 of DESIGN.md.
+//
+//   L0 preprocess_kernel   flux, flux_err -> (w f, w) float2, zero outside the data
+//   L1 build_taps_kernel   per duration: nearest-neighbour template samples m, m^2     (R3)
+//   L2 linear_search_kernel  S_wmf = sum m (w f), S_wmm = sum m^2 w for every (t_i, D_j)
+//   L3 (fused epilogue)    depth = S_wmf/S_wmm, var = 1/S_wmm, dlogL = 1/2 S_wmf^2/S_wmm (Eq. 2)
+//
+// The windowed sums are a correlation of the sample stream with 2H_j+1 taps.  For a t0 stride of q
+// samples the taps are split into q polyphase sub-filters, so that R consecutive outputs of one
+// thread slide over a register window: one 8-byte shared-memory load feeds 2R FFMAs.
+#include "linear_search.cuh"
+
+#include <math.h>
+
+#include <algorithm>
+#include <vector>
+
+namespace cetra {
+
+// ------------------------------------------------------------------------------------------- L0
+template <typename T>
+__global__ void preprocess_kernel(const T *__restrict__ flux, const T *__restrict__ flux_err, long long n,
+                                  long long n_lc, float2 *__restrict__ wfw, long long row_len, long long n_lo) {
+    const long long total = n_lc * row_len;
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
+         idx += (long long)gridDim.x * blockDim.x) {
+        const long long lc = idx / row_len;
+        const long long nn = idx - lc * row_len + n_lo;
+        float2 out = make_float2(0.f, 0.f);
+        if (nn >= 0 && nn < n) {
+            const T fl = flux[lc * n + nn];
+            const T er = flux_err[lc * n + nn];
+            if (isfinite(fl) && isfinite(er) && er > T(0)) {      // null points carry no weight
+                const T f = T(1) - fl;                            // offset from baseline, dips positive
+                const T w = T(1) / (er * er);
+                const float wf32 = static_cast<float>(w * f);
+                const float w32 = static_cast<float>(w);
+                if (isfinite(wf32) && isfinite(w32)) out = make_float2(wf32, w32);
+            }
+        }
+        wfw[idx] = out;
+    }
+}
+
+// ------------------------------------------------------------------------------------------- L1
+// One thread per stored tap.  Layout per duration j: [q phases][A_j taps] float2 (m, m^2), tap (b, a) is the
+// sample offset k = q*a + b - H_j from the window centre; zero beyond the window.  Every FP64 step is an
+// explicitly rounded IEEE operation so that the index agrees bit for bit with a plain CPU evaluation (R3).
+__global__ void build_taps_kernel(const __grid_constant__ LinearParams P, const float *__restrict__ tpl,
+                                  int n_tpl, double cadence, float2 *__restrict__ taps) {
+    const int j = blockIdx.y;
+    const int A = P.A[j], H = P.H[j], q = P.q;
+    const int stored = P.tap_off[j + 1] - P.tap_off[j];
+    const double D = P.durations[j];
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < stored; idx += gridDim.x * blockDim.x) {
+        float m = 0.f;
+        if (idx < q * A) {
+            const int b = idx / A, a = idx - b * A;
+            const int kk = q * a + b;
+            if (kk <= 2 * H) {
+                const double k = static_cast<double>(kk - H);
+                const double x = __dadd_rn(__ddiv_rn(__dmul_rn(k, cadence), D), 0.5);
+                if (x >= 0.0 && x <= 1.0) {
+                    const double pos = __dadd_rn(__dmul_rn(x, static_cast<double>(n_tpl - 1)), 0.5);
+                    m = tpl[static_cast<int>(floor(pos))];
+                }
+            }
+        }
+        taps[P.tap_off[j] + idx] = make_float2(m, m * m);
+    }
+}
+
+// ------------------------------------------------------------------------------------------- L2 + L3
+template <int R, int WARPS, bool Q1>
+__global__ void __launch_bounds__(WARPS * 32)
+linear_search_kernel(const __grid_constant__ LinearParams P) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    constexpr int TILE = WARPS * 32 * R;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+
+    const int per_lc = P.tiles_per_row * P.n_dur;
+    const long long lc = blockIdx.x / per_lc;
+    const int rem = static_cast<int>(blockIdx.x - lc * per_lc);
+    const int j = P.order[rem / P.tiles_per_row];               // longest durations first
+    const int tile = rem % P.tiles_per_row;
+    const int q = Q1 ? 1 : P.q;
+    const int A = P.A[j];
+    const long long i_blk = static_cast<long long>(tile) * TILE;
+
+    // sample range of this tile in the padded (w f, w) row: starts at the first tap of the first output
+    const long long s_first = P.n0 - P.H[j] + q * i_blk - P.n_lo;
+    const int d0 = static_cast<int>(s_first & 1);                // bulk copies need 16-byte alignment
+    const int len = (d0 + q * (TILE + A) + 1) & ~1;
+    const int n_tap = P.tap_off[j + 1] - P.tap_off[j];
+
+    uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
+    float2 *data = reinterpret_cast<float2 *>(smem_raw + 16);
+    float2 *taps = data + len;
+    float2 *stage = taps + n_tap;
+
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (tid == 0) {
+        const uint32_t bytes_data = static_cast<uint32_t>(len) * 8u, bytes_taps = static_cast<uint32_t>(n_tap) * 8u;
+        mbar_arrive_expect_tx(bar, bytes_data + bytes_taps);
+        bulk_copy_g2s_chunked(data, P.wfw + lc * P.lc_pitch + (s_first - d0), bytes_data, bar);
+        bulk_copy_g2s_chunked(taps, P.taps + P.tap_off[j], bytes_taps, bar);
+    }
+    mbar_wait(bar, 0);
+
+    float accA[R], accB[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) { accA[r] = 0.f; accB[r] = 0.f; }
+
+    const float2 *xs = data + d0 + q * (tid * R);
+    for (int b = 0; b < q; ++b) {
+        const float2 *xb = xs + b;
+        const float2 *tb = taps + b * A;
+        float2 win[R];
+#pragma unroll
+        for (int v = 0; v < R - 1; ++v) win[v] = xb[q * v];
+        float2 nxt = xb[q * (R - 1)];
+        float2 tap = tb[0];
+        const float2 *xp = xb + q * R;
+        for (int a0 = 0; a0 < A; a0 += R) {
+#pragma unroll
+            for (int u = 0; u < R; ++u) {
+                win[(u + R - 1) % R] = nxt;
+                const float2 t = tap;
+                nxt = Q1 ? xp[u] : *xp;                          // prefetch the next window element
+                if (!Q1) xp += q;
+                tap = tb[a0 + u + 1];
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const float2 x = win[(u + r) % R];
+                    accB[r] = fmaf(t.x, x.x, accB[r]);           // S_wmf += m   * (w f)
+                    accA[r] = fmaf(t.y, x.y, accA[r]);           // S_wmm += m^2 * w
+                }
+            }
+            if (Q1) xp += R;
+        }
+    }
+
+    // transpose through shared memory so that the global stores are coalesced
+    float2 *st = stage + warp * (32 * R);
+#pragma unroll
+    for (int r = 0; r < R; ++r) st[lane * R + r] = make_float2(accA[r], accB[r]);
+    __syncwarp();
+    const long long row = lc * P.n_dur + j;
+    const long long i_warp = i_blk + static_cast<long long>(warp) * (32 * R);
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const long long i = i_warp + r * 32 + lane;
+        if (i < P.n_t0) {
+            const float2 ab = st[r * 32 + lane];
+            const float a = ab.x, bsum = ab.y;
+            const bool null_cell = !(a > 0.f);                  // no observation in the window
+            const float nanv = __int_as_float(0x7fc00000);
+            const float depth = null_cell ? nanv : bsum / a;
+            if (P.depth) P.depth[row * P.n_t0 + i] = depth;
+            if (P.var) P.var[row * P.n_t0 + i] = null_cell ? nanv : 1.0f / a;
+            if (P.dlogL) P.dlogL[row * P.n_t0 + i] = null_cell ? nanv : 0.5f * bsum * depth;
+            if (P.stats) P.stats[row * P.stats_pitch + i] = null_cell ? make_float2(0.f, 0.f) : ab;
+        }
+    }
+    if (P.stats && tile == P.tiles_per_row - 1) {               // zero the row padding
+        for (long long i = P.n_t0 + tid; i < P.stats_pitch; i += WARPS * 32)
+            P.stats[row * P.stats_pitch + i] = make_float2(0.f, 0.f);
+    }
+}
+
+// ------------------------------------------------------------------------------------------- host
+static size_t linear_smem_bytes(const LinearPlan &pl, int R, int warps) {
+    const int tile = warps * 32 * R;
+    size_t worst = 0;
+    for (int j = 0; j < pl.P.n_dur; ++j) {
+        const size_t len = (static_cast<size_t>(1 + pl.P.q * (tile + pl.P.A[j]) + 1)) & ~size_t(1);
+        const size_t n_tap = pl.P.tap_off[j + 1] - pl.P.tap_off[j];
+        worst = std::max(worst, 16 + (len + n_tap + tile) * 8);
+    }
+    return worst;
+}
+
+int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const double *durations_host,
+                      int32_t n_dur, cetra_t0_grid grid, int32_t n_template, int smem_limit, int n_sm,
+                      LinearPlan *pl) {
+    if (!times_host || !durations_host || n < 2 || n_lc < 1 || n_dur < 1 || grid.n_t0 < 1 || n_template < 2)
+        return CETRA_ERR_INVALID_ARG;
+    if (n_dur > CETRA_MAX_DURATIONS) return CETRA_ERR_UNSUPPORTED;
+    int rc = derive_geometry(times_host, n, grid, &pl->geo);
+    if (rc != CETRA_OK) return rc;
+    if (pl->geo.q > (1 << 20)) return CETRA_ERR_UNSUPPORTED;
+    LinearParams &P = pl->P;
+    constexpr int R = kLinearR;
+    P.q = static_cast<int>(pl->geo.q);
+    P.n0 = pl->geo.n0;
+    P.n_t0 = grid.n_t0;
+    P.n_dur = n_dur;
+    int h_max = 0, a_max = 0;
+    P.tap_off[0] = 0;
+    for (int j = 0; j < n_dur; ++j) {
+        const double D = durations_host[j];
+        if (!(D > 0.0) || !std::isfinite(D)) return CETRA_ERR_INVALID_ARG;
+        const double h = floor(D / (2.0 * pl->geo.cadence)) + 1.0;     // safe superset of the window (R2)
+        if (h > 4.0e6) return CETRA_ERR_UNSUPPORTED;
+        P.H[j] = static_cast<int>(h);
+        const int ntap = 2 * P.H[j] + 1;
+        const int per_phase = (ntap + P.q - 1) / P.q;
+        P.A[j] = (per_phase + R - 1) / R * R;
+        P.durations[j] = D;
+        const long long stored = (static_cast<long long>(P.q) * P.A[j] + 2 + 1) & ~1LL;   // +2: prefetch overrun
+        if (P.tap_off[j] + stored > 0x7fffffffLL) return CETRA_ERR_UNSUPPORTED;
+        P.tap_off[j + 1] = static_cast<int>(P.tap_off[j] + stored);
+        h_max = std::max(h_max, P.H[j]);
+        a_max = std::max(a_max, P.A[j]);
+    }
+    pl->taps_total = P.tap_off[n_dur];
+    // durations by decreasing cost, so that the heavy blocks are scheduled first
+    std::vector<int> ord(n_dur);
+    for (int j = 0; j < n_dur; ++j) ord[j] = j;
+    std::stable_sort(ord.begin(), ord.end(), [&](int a, int b) { return P.A[a] > P.A[b]; });
+    for (int j = 0; j < n_dur; ++j) P.order[j] = static_cast<unsigned char>(ord[j]);
+
+    // tile shape: as many warps per block as shared memory allows, fewer when the grid would not fill the chip
+    int warps = 4;
+    for (;;) {
+        const int tile = warps * 32 * R;
+        const long long tiles = (grid.n_t0 + tile - 1) / tile;
+        const long long blocks = tiles * n_dur * n_lc;
+        const bool fits = linear_smem_bytes(*pl, R, warps) <= static_cast<size_t>(smem_limit);
+        if (warps == 1 || (fits && blocks >= 2LL * n_sm)) {
+            if (!fits) return CETRA_ERR_UNSUPPORTED;
+            break;
+        }
+        warps /= 2;
+    }
+    pl->warps = warps;
+    pl->tile = warps * 32 * R;
+    P.tiles_per_row = static_cast<int>((grid.n_t0 + pl->tile - 1) / pl->tile);
+    if (static_cast<long long>(P.tiles_per_row) * n_dur * n_lc > 0x7fffffffLL) return CETRA_ERR_UNSUPPORTED;
+    pl->smem_bytes = linear_smem_bytes(*pl, R, warps);
+
+    // padded (w f, w) row: sample index n_lo is element 0
+    P.n_lo = P.n0 - h_max - 2;
+    const long long n_hi = P.n0 + static_cast<long long>(P.q) * (static_cast<long long>(P.tiles_per_row) * pl->tile + a_max) + P.q + 4;
+    P.lc_pitch = round_up64(n_hi - P.n_lo, 4);
+    P.stats_pitch = cetra_stats_pitch(grid.n_t0);
+    return CETRA_OK;
+}
+
+size_t linear_workspace_bytes(const LinearPlan &pl, int32_t n_lc, int32_t n_template) {
+    size_t b = 0;
+    b += align_up(sizeof(float2) * static_cast<size_t>(pl.P.lc_pitch) * n_lc);   // (w f, w)
+    b += align_up(sizeof(float2) * static_cast<size_t>(pl.taps_total));          // taps
+    b += align_up(sizeof(float) * static_cast<size_t>(n_template));              // template
+    return b;
+}
+
+template <int R, int WARPS>
+static int launch_linear(const LinearPlan &pl, const LinearParams &P, long long blocks, cudaStream_t st) {
+    if (P.q == 1) {
+        auto k = linear_search_kernel<R, WARPS, true>;
+        CETRA_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes));
+        k<<<static_cast<unsigned>(blocks), WARPS * 32, pl.smem_bytes, st>>>(P);
+    } else {
+        auto k = linear_search_kernel<R, WARPS, false>;
+        CETRA_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes));
+        k<<<static_cast<unsigned>(blocks), WARPS * 32, pl.smem_bytes, st>>>(P);
+    }
+    CETRA_LAUNCH_CHECK();
+    return CETRA_OK;
+}
+
+int run_linear(LinearPlan &pl, const void *flux_dev, const void *flux_err_dev, cetra_dtype dtype, int64_t n,
+               int32_t n_lc, const float *template_host, int32_t n_template, bool template_on_device,
+               float *depth_dev, float *var_dev, float *dlogL_dev, float *stats_dev, void *workspace_dev,
+               cudaStream_t st) {
+    Carver ws(workspace_dev);
+    float2 *wfw = ws.take<float2>(static_cast<size_t>(pl.P.lc_pitch) * n_lc);
+    float2 *taps = ws.take<float2>(static_cast<size_t>(pl.taps_total));
+    float *tpl = ws.take<float>(static_cast<size_t>(n_template));
+    LinearParams &P = pl.P;
+    P.wfw = wfw;
+    P.taps = taps;
+    P.depth = depth_dev; P.var = var_dev; P.dlogL = dlogL_dev;
+    P.stats = reinterpret_cast<float2 *>(stats_dev);
+
+    if (!pl.taps_ready) {
+        if (template_on_device) {
+            CETRA_CUDA_TRY(cudaMemcpyAsync(tpl, template_host, sizeof(float) * n_template, cudaMemcpyDeviceToDevice, st));
+        } else {
+            CETRA_CUDA_TRY(cudaMemcpyAsync(tpl, template_host, sizeof(float) * n_template, cudaMemcpyHostToDevice, st));
+        }
+        int max_stored = 0;
+        for (int j = 0; j < P.n_dur; ++j) max_stored = std::max(max_stored, P.tap_off[j + 1] - P.tap_off[j]);
+        dim3 g((max_stored + 255) / 256, P.n_dur);
+        build_taps_kernel<<<g, 256, 0, st>>>(P, tpl, n_template, pl.geo.cadence, taps);
+        CETRA_LAUNCH_CHECK();
+        pl.taps_ready = true;
+    }
+    {
+        const long long total = static_cast<long long>(n_lc) * P.lc_pitch;
+        const int blocks = static_cast<int>(std::min<long long>((total + 255) / 256, 148LL * 16));
+        if (dtype == CETRA_F32)
+            preprocess_kernel<float><<<blocks, 256, 0, st>>>(static_cast<const float *>(flux_dev),
+                                                            static_cast<const float *>(flux_err_dev), n, n_lc, wfw,
+                                                            P.lc_pitch, P.n_lo);
+        else
+            preprocess_kernel<double><<<blocks, 256, 0, st>>>(static_cast<const double *>(flux_dev),
+                                                             static_cast<const double *>(flux_err_dev), n, n_lc, wfw,
+                                                             P.lc_pitch, P.n_lo);
+        CETRA_LAUNCH_CHECK();
+    }
+    const long long blocks = static_cast<long long>(P.tiles_per_row) * P.n_dur * n_lc;
+    constexpr int R = kLinearR;
+    switch (pl.warps) {
+        case 4: return launch_linear<R, 4>(pl, P, blocks, st);
+        case 2: return launch_linear<R, 2>(pl, P, blocks, st);
+        default: return launch_linear<R, 1>(pl, P, blocks, st);
+    }
+}
+
+}  // namespace cetra

@@ -1,0 +1,43 @@
+// Host-side plan and kernel parameters of the linear search (§2.2).
+#pragma once
+
+#include "common.cuh"
+
+namespace cetra {
+
+constexpr int kLinearR = 15;   // consecutive t0 cells per thread; odd => conflict-free 8-byte shared loads
+
+// Passed by value (__grid_constant__): no device copy, no host synchronisation.
+struct LinearParams {
+    const float2 *wfw;          // [n_lc][lc_pitch] (w f, w), element 0 is sample index n_lo
+    const float2 *taps;         // per duration [q][A_j] (m, m^2), see build_taps_kernel
+    float *depth, *var, *dlogL; // [n_lc][n_dur][n_t0] or null
+    float2 *stats;              // [n_lc][n_dur][stats_pitch] or null
+    long long lc_pitch, n_lo, n0, n_t0, stats_pitch;
+    int q, n_dur, tiles_per_row;
+    int H[CETRA_MAX_DURATIONS];         // window half-reach in samples (superset of the window)
+    int A[CETRA_MAX_DURATIONS];         // taps per polyphase branch, padded to a multiple of kLinearR
+    int tap_off[CETRA_MAX_DURATIONS + 1];
+    unsigned char order[CETRA_MAX_DURATIONS];
+    double durations[CETRA_MAX_DURATIONS];
+};
+
+struct LinearPlan {
+    Geometry geo;
+    LinearParams P{};
+    int warps = 0, tile = 0;
+    long long taps_total = 0;
+    size_t smem_bytes = 0;
+    bool taps_ready = false;    // tap tables already built in this workspace (batched path re-uses them)
+};
+
+int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const double *durations_host,
+                      int32_t n_dur, cetra_t0_grid grid, int32_t n_template, int smem_limit, int n_sm,
+                      LinearPlan *pl);
+size_t linear_workspace_bytes(const LinearPlan &pl, int32_t n_lc, int32_t n_template);
+int run_linear(LinearPlan &pl, const void *flux_dev, const void *flux_err_dev, cetra_dtype dtype, int64_t n,
+               int32_t n_lc, const float *template_host, int32_t n_template, bool template_on_device,
+               float *depth_dev, float *var_dev, float *dlogL_dev, float *stats_dev, void *workspace_dev,
+               cudaStream_t st);
+
+}  // namespace cetra

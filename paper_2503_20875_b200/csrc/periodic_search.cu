@@ -1,0 +1,327 @@
+// Periodic search (§2.3): steps P1-P4 of DESIGN.md.
+//
+//   P1 epoch offsets        off_e = llrint(e * P_k / stride) in FP64, 32 epochs per warp at a time (R11)
+//   P2 fold-gather-sum      SA = sum_e S_wmm[j][p + off_e], SB = sum_e S_wmf[j][p + off_e]
+//   P3 combine              Z = SB/SA, var = 1/SA, LR = 1/2 SB^2/SA  (= Eq. 4 summed at Z)
+//   P4 argmax               per period: max LR over (duration, phase), ties -> smallest j, then p
+//
+// The combined (depth, var, LR) arrays of a period are never materialised: a warp folds one
+// (period, duration) pair in registers and publishes one packed 64-bit key with atomicMax.
+// A block keeps the (S_wmm, S_wmf) row of one duration in shared memory (one TMA bulk copy per row)
+// and pulls (row, period-segment) work items from a global queue; rows that do not fit in shared
+// memory are gathered from L2 with coalesced read-only loads.
+#include "periodic_search.cuh"
+
+#include <math.h>
+
+#include <algorithm>
+
+namespace cetra {
+
+__device__ __forceinline__ float2 add2(float2 a, float2 b) {
+    // packed FP32 add (FADD2 on sm_100a): one issue slot for both sufficient statistics
+    float2 r;
+    asm("{\n\t"
+        ".reg .b64 ra, rb, rc;\n\t"
+        "mov.b64 ra, {%2, %3};\n\t"
+        "mov.b64 rb, {%4, %5};\n\t"
+        "add.rn.f32x2 rc, ra, rb;\n\t"
+        "mov.b64 {%0, %1}, rc;\n\t"
+        "}"
+        : "=f"(r.x), "=f"(r.y)
+        : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return r;
+}
+
+__device__ __forceinline__ float rcp_approx(float x) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+template <bool kSmemRow>
+__device__ __forceinline__ float2 load_cell(const float2 *p) {
+    if (kSmemRow) return *p;
+    return __ldg(p);
+}
+
+// One pass of a warp over G*32 consecutive phases starting at p0: lane handles phases p0 + lane + 32 g.
+// Cells beyond n_t0-1 are zero (row padding), so epochs that run off the end for the later phases of the
+// pass add nothing; the epoch loop itself stops at the last epoch valid for p0.
+template <int G, bool kSmemRow>
+__device__ __forceinline__ void fold_pass(const float2 *__restrict__ row, int p0, int n_t0, int n_phase, double r,
+                                          int lane, float &best_lr, int &best_p) {
+    float2 acc[G];
+#pragma unroll
+    for (int g = 0; g < G; ++g) acc[g] = make_float2(0.f, 0.f);
+    const long long limit = static_cast<long long>(n_t0) - 1 - p0;     // off_e <= limit  <=>  p0 + off_e <= I-1
+    const float2 *base = row + p0 + lane;
+    for (int eb = 0;; eb += 32) {
+        const long long off_ll = __double2ll_rn(__dmul_rn(static_cast<double>(eb + lane), r));   // R11
+        const bool ok = off_ll <= limit;
+        const int my_off = ok ? static_cast<int>(off_ll) : 0;
+        const int cnt = __popc(__ballot_sync(0xffffffffu, ok));      // offsets are monotone in e: valid ones are a prefix
+#pragma unroll 4
+        for (int t = 0; t < cnt; ++t) {
+            const int off = __shfl_sync(0xffffffffu, my_off, t);
+            const float2 *ptr = base + off;
+#pragma unroll
+            for (int g = 0; g < G; ++g) acc[g] = add2(acc[g], load_cell<kSmemRow>(ptr + 32 * g));
+        }
+        if (cnt < 32) break;
+    }
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+        const int p = p0 + lane + 32 * g;
+        const float a = acc[g].x, b = acc[g].y;
+        // candidate iff some epoch contributed (S_wmm > 0); selection uses an approximate reciprocal,
+        // the reported values are recomputed with IEEE division by finalize_peaks_kernel
+        const float lr = 0.5f * b * b * rcp_approx(a);
+        if (p < n_phase && a > 0.f && lr > best_lr) { best_lr = lr; best_p = p; }
+    }
+}
+
+template <bool kSmemRow>
+__device__ __forceinline__ void fold_period(const float2 *__restrict__ row, int n_t0, double r, int n_phase, int lane,
+                                            float &best_lr, int &best_p) {
+    best_lr = -1.f;
+    best_p = 0x7fffffff;
+    int p0 = 0;
+    for (; p0 + 32 * kFoldR <= n_phase; p0 += 32 * kFoldR)
+        fold_pass<kFoldR, kSmemRow>(row, p0, n_t0, n_phase, r, lane, best_lr, best_p);
+    const int groups = (n_phase - p0 + 31) >> 5;
+    switch (groups) {
+        case 1: fold_pass<1, kSmemRow>(row, p0, n_t0, n_phase, r, lane, best_lr, best_p); break;
+        case 2: fold_pass<2, kSmemRow>(row, p0, n_t0, n_phase, r, lane, best_lr, best_p); break;
+        case 3: fold_pass<3, kSmemRow>(row, p0, n_t0, n_phase, r, lane, best_lr, best_p); break;
+        default: break;
+    }
+    // warp argmax: larger lr wins, ties -> smaller phase
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) {
+        const float o_lr = __shfl_xor_sync(0xffffffffu, best_lr, s);
+        const int o_p = __shfl_xor_sync(0xffffffffu, best_p, s);
+        if (o_lr > best_lr || (o_lr == best_lr && o_p < best_p)) { best_lr = o_lr; best_p = o_p; }
+    }
+}
+
+template <bool kSmemRow>
+__global__ void __launch_bounds__(kFoldThreads, 1) fold_argmax_kernel(const __grid_constant__ PeriodicParams P) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
+    unsigned int *s_seg = reinterpret_cast<unsigned int *>(smem_raw + 8);
+    float2 *srow = reinterpret_cast<float2 *>(smem_raw + 16);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int kWarps = kFoldThreads / 32;
+
+    if (kSmemRow && tid == 0) {
+        mbar_init(bar, 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    long long cur_row = -1;
+    uint32_t parity = 0;
+    for (;;) {
+        if (tid == 0) *s_seg = atomicAdd(P.counter, 1u);
+        __syncthreads();
+        const long long seg = *s_seg;
+        __syncthreads();                       // everyone has read the slot and is done with the previous row
+        if (seg >= P.n_segs) break;
+        const long long rowid = seg / P.segs_per_row;              // lc * n_dur + j
+        const int s = static_cast<int>(seg - rowid * P.segs_per_row);
+        const int j = static_cast<int>(rowid % P.n_dur);
+        const long long lc = rowid / P.n_dur;
+        const float2 *grow = P.stats + rowid * P.stats_pitch;
+        if (kSmemRow && rowid != cur_row) {
+            if (tid == 0) {
+                const uint32_t bytes = static_cast<uint32_t>(P.stats_pitch) * 8u;
+                mbar_arrive_expect_tx(bar, bytes);
+                bulk_copy_g2s_chunked(srow, grow, bytes, bar);
+            }
+            mbar_wait(bar, parity);
+            parity ^= 1u;
+            cur_row = rowid;
+        }
+        const float2 *row = kSmemRow ? srow : grow;
+        const double D = P.durations[j];
+        const int k_end = min(P.n_per, (s + 1) * P.seg_len);
+        for (int k = s * P.seg_len + warp; k < k_end; k += kWarps) {
+            const double period = P.periods[k];
+            if (!(D < period)) continue;                            // overlapping windows are invalid
+            if (P.dur_lo && (j < P.dur_lo[k] || j >= P.dur_hi[k])) continue;
+            const double r = __ddiv_rn(period, P.t0_stride);        // period in t0 cells, FP64 (R11)
+            const double rc = ceil(r);
+            const int n_phase = rc < static_cast<double>(P.n_t0) ? static_cast<int>(rc) : P.n_t0;   // R10
+            float best_lr;
+            int best_p;
+            fold_period<kSmemRow>(row, P.n_t0, r, n_phase, lane, best_lr, best_p);
+            if (lane == 0 && best_lr >= 0.f) {
+                const unsigned int id = static_cast<unsigned int>(j) * static_cast<unsigned int>(P.n_t0) +
+                                        static_cast<unsigned int>(best_p);
+                const unsigned long long key =
+                    (static_cast<unsigned long long>(__float_as_uint(best_lr)) << 32) | (0xffffffffu - id);
+                atomicMax(P.keys + lc * P.n_per + k, key);
+            }
+        }
+    }
+}
+
+// One thread per (light curve, period): decode the winning (j, p), redo its fold in the same order with
+// IEEE division, count the contributing epochs and write the record.
+__global__ void finalize_peaks_kernel(const __grid_constant__ PeriodicParams P, cetra_peak *__restrict__ peaks) {
+    const long long total = static_cast<long long>(P.n_lc) * P.n_per;
+    for (long long idx = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; idx < total;
+         idx += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const unsigned long long key = P.keys[idx];
+        cetra_peak out;
+        const float nanv = __int_as_float(0x7fc00000);
+        out.lr = nanv; out.depth = nanv; out.depth_var = nanv; out.t0 = nanv;
+        out.i_t0 = -1; out.j_dur = -1; out.n_transits = 0; out.reserved = 0;
+        if (key != 0ull) {
+            const long long lc = idx / P.n_per;
+            const int k = static_cast<int>(idx - lc * P.n_per);
+            const unsigned int id = 0xffffffffu - static_cast<unsigned int>(key & 0xffffffffull);
+            const int j = static_cast<int>(id / static_cast<unsigned int>(P.n_t0));
+            const int p = static_cast<int>(id - static_cast<unsigned int>(j) * static_cast<unsigned int>(P.n_t0));
+            const float2 *row = P.stats + (lc * P.n_dur + j) * P.stats_pitch;
+            const double r = __ddiv_rn(P.periods[k], P.t0_stride);
+            float sa = 0.f, sb = 0.f;
+            int ntr = 0;
+            for (long long e = 0;; ++e) {
+                const long long cell = p + __double2ll_rn(__dmul_rn(static_cast<double>(e), r));
+                if (cell > P.n_t0 - 1) break;
+                const float2 ab = row[cell];
+                sa += ab.x;
+                sb += ab.y;
+                ntr += ab.x > 0.f ? 1 : 0;
+            }
+            out.depth = sb / sa;                                     // common depth Z
+            out.depth_var = 1.0f / sa;
+            out.lr = 0.5f * sb * out.depth;
+            out.t0 = static_cast<float>(P.t0_start + static_cast<double>(p) * P.t0_stride);
+            out.i_t0 = p; out.j_dur = j; out.n_transits = ntr;
+        }
+        peaks[idx] = out;
+    }
+}
+
+// (depth, var) grids -> (S_wmm, S_wmf) rows: S_wmm = 1/var, S_wmf = depth/var, null (NaN) cells -> 0.
+__global__ void grids_to_stats_kernel(const float *__restrict__ depth, const float *__restrict__ var, long long n_rows,
+                                      long long n_t0, long long pitch, float2 *__restrict__ stats) {
+    const long long total = n_rows * pitch;
+    for (long long idx = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; idx < total;
+         idx += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const long long rowid = idx / pitch;
+        const long long i = idx - rowid * pitch;
+        float2 out = make_float2(0.f, 0.f);
+        if (i < n_t0) {
+            const float d = depth[rowid * n_t0 + i], v = var[rowid * n_t0 + i];
+            if (isfinite(d) && isfinite(v) && v > 0.f) {
+                const float a = 1.0f / v;
+                const float b = d / v;
+                if (isfinite(a) && isfinite(b)) out = make_float2(a, b);
+            }
+        }
+        stats[idx] = out;
+    }
+}
+
+// ------------------------------------------------------------------------------------------- host
+int build_periodic_plan(int32_t n_lc, int32_t n_dur, cetra_t0_grid grid, const double *durations_host,
+                        const double *periods_host, int32_t n_per, int smem_limit, int n_sm, PeriodicPlan *pl) {
+    if (!durations_host || !periods_host || n_lc < 1 || n_dur < 1 || n_per < 1 || grid.n_t0 < 1 ||
+        !(grid.t0_stride > 0.0) || !std::isfinite(grid.t0_stride) || !std::isfinite(grid.t0_start))
+        return CETRA_ERR_INVALID_ARG;
+    if (n_dur > CETRA_MAX_DURATIONS) return CETRA_ERR_UNSUPPORTED;
+    // the packed cell id (j * n_t0 + p) must fit 32 bits, cell indices an int
+    if (grid.n_t0 > 0x7fffffffLL - 4096 || static_cast<long long>(n_dur) * grid.n_t0 >= 0xffffffffLL)
+        return CETRA_ERR_UNSUPPORTED;
+    for (int k = 0; k < n_per; ++k)
+        if (!(periods_host[k] >= grid.t0_stride) || !std::isfinite(periods_host[k])) return CETRA_ERR_INVALID_ARG;
+    PeriodicParams &P = pl->P;
+    for (int j = 0; j < n_dur; ++j) {
+        if (!(durations_host[j] > 0.0) || !std::isfinite(durations_host[j])) return CETRA_ERR_INVALID_ARG;
+        P.durations[j] = durations_host[j];
+    }
+    P.n_lc = n_lc; P.n_dur = n_dur; P.n_t0 = static_cast<int>(grid.n_t0); P.n_per = n_per;
+    P.t0_start = grid.t0_start; P.t0_stride = grid.t0_stride;
+    P.stats_pitch = cetra_stats_pitch(grid.n_t0);
+    const size_t row_bytes = static_cast<size_t>(P.stats_pitch) * sizeof(float2);
+    pl->row_in_smem = row_bytes + 16 <= static_cast<size_t>(smem_limit);
+    pl->smem_bytes = pl->row_in_smem ? row_bytes + 16 : 16;
+    // period segments: a multiple of the warps per block so that every warp folds the same number of
+    // periods; shorter segments when the problem would otherwise not fill the chip
+    const long long rows = static_cast<long long>(n_lc) * n_dur;
+    constexpr int kWarps = kFoldThreads / 32;
+    int seg_len = 4 * kWarps;
+    while (seg_len > kWarps && rows * ((n_per + seg_len - 1) / seg_len) < 8LL * n_sm) seg_len /= 2;
+    P.seg_len = seg_len;
+    P.segs_per_row = (n_per + seg_len - 1) / seg_len;
+    P.n_segs = rows * P.segs_per_row;
+    if (P.n_segs > 0x7fffffffLL - 4096) return CETRA_ERR_UNSUPPORTED;
+    const int per_sm = (pl->smem_bytes * 2 + 2048 <= static_cast<size_t>(smem_limit)) ? 2 : 1;
+    pl->grid = static_cast<int>(std::min<long long>(P.n_segs, static_cast<long long>(n_sm) * per_sm));
+    return CETRA_OK;
+}
+
+size_t periodic_workspace_bytes(int32_t n_lc, int32_t n_per) {
+    size_t b = 0;
+    b += align_up(sizeof(double) * static_cast<size_t>(n_per));                           // periods
+    b += 2 * align_up(sizeof(int) * static_cast<size_t>(n_per));                          // dur_lo, dur_hi
+    b += align_up(sizeof(unsigned long long) * static_cast<size_t>(n_lc) * n_per + 256);  // keys + counter
+    return b;
+}
+
+int run_periodic(PeriodicPlan &pl, const float2 *stats_dev, const double *periods_host, const int32_t *dur_lo_host,
+                 const int32_t *dur_hi_host, bool upload, cetra_peak *peaks_dev, void *workspace_dev,
+                 cudaStream_t st) {
+    PeriodicParams &P = pl.P;
+    Carver ws(workspace_dev);
+    double *periods = ws.take<double>(P.n_per);
+    int *lo = ws.take<int>(P.n_per);
+    int *hi = ws.take<int>(P.n_per);
+    const size_t n_keys = static_cast<size_t>(P.n_lc) * P.n_per;
+    unsigned long long *keys = ws.take<unsigned long long>(n_keys + 32);
+    const bool ranges = dur_lo_host && dur_hi_host;
+    if (upload) {
+        CETRA_CUDA_TRY(cudaMemcpyAsync(periods, periods_host, sizeof(double) * P.n_per, cudaMemcpyHostToDevice, st));
+        if (ranges) {
+            CETRA_CUDA_TRY(cudaMemcpyAsync(lo, dur_lo_host, sizeof(int) * P.n_per, cudaMemcpyHostToDevice, st));
+            CETRA_CUDA_TRY(cudaMemcpyAsync(hi, dur_hi_host, sizeof(int) * P.n_per, cudaMemcpyHostToDevice, st));
+        }
+    }
+    P.stats = stats_dev;
+    P.periods = periods;
+    P.dur_lo = ranges ? lo : nullptr;
+    P.dur_hi = ranges ? hi : nullptr;
+    P.keys = keys;
+    P.counter = reinterpret_cast<unsigned int *>(keys + n_keys);
+    CETRA_CUDA_TRY(cudaMemsetAsync(keys, 0, sizeof(unsigned long long) * (n_keys + 32), st));
+    if (pl.row_in_smem) {
+        auto k = fold_argmax_kernel<true>;
+        CETRA_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes));
+        k<<<pl.grid, kFoldThreads, pl.smem_bytes, st>>>(P);
+    } else {
+        fold_argmax_kernel<false><<<pl.grid, kFoldThreads, pl.smem_bytes, st>>>(P);
+    }
+    CETRA_LAUNCH_CHECK();
+    {
+        const long long total = static_cast<long long>(P.n_lc) * P.n_per;
+        const int blocks = static_cast<int>(std::min<long long>((total + 255) / 256, 148LL * 8));
+        finalize_peaks_kernel<<<blocks, 256, 0, st>>>(P, peaks_dev);
+        CETRA_LAUNCH_CHECK();
+    }
+    return CETRA_OK;
+}
+
+int run_grids_to_stats(const float *depth_dev, const float *var_dev, int32_t n_rows, int64_t n_t0,
+                       float2 *stats_dev, cudaStream_t st) {
+    const long long pitch = cetra_stats_pitch(n_t0);
+    const long long total = static_cast<long long>(n_rows) * pitch;
+    const int blocks = static_cast<int>(std::min<long long>((total + 255) / 256, 148LL * 16));
+    grids_to_stats_kernel<<<blocks, 256, 0, st>>>(depth_dev, var_dev, n_rows, n_t0, pitch, stats_dev);
+    CETRA_LAUNCH_CHECK();
+    return CETRA_OK;
+}
+
+}  // namespace cetra

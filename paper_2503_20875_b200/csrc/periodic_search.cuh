@@ -1,0 +1,42 @@
+// Host-side plan and kernel parameters of the periodic search (§2.3).
+#pragma once
+
+#include "common.cuh"
+
+namespace cetra {
+
+constexpr int kFoldR = 4;            // phase groups (of 32 phases) per warp pass; needs kStatsPad >= 32*kFoldR
+constexpr int kFoldThreads = 1024;
+
+struct PeriodicParams {
+    const float2 *stats;             // [n_lc][n_dur][stats_pitch] (S_wmm, S_wmf), zero in null cells / padding
+    const double *periods;           // [n_per] device
+    const int *dur_lo, *dur_hi;      // [n_per] device or null
+    unsigned long long *keys;        // [n_lc][n_per] packed (lr bits << 32 | ~cell id), 0 = no candidate
+    unsigned int *counter;           // segment queue head
+    long long stats_pitch;
+    double t0_start, t0_stride;
+    int n_lc, n_dur, n_t0, n_per;
+    int segs_per_row, seg_len;
+    long long n_segs;
+    double durations[CETRA_MAX_DURATIONS];
+};
+
+struct PeriodicPlan {
+    PeriodicParams P{};
+    bool row_in_smem = false;
+    size_t smem_bytes = 0;
+    int grid = 0;
+};
+
+int build_periodic_plan(int32_t n_lc, int32_t n_dur, cetra_t0_grid grid, const double *durations_host,
+                        const double *periods_host, int32_t n_per, int smem_limit, int n_sm, PeriodicPlan *pl);
+size_t periodic_workspace_bytes(int32_t n_lc, int32_t n_per);   // periods, ranges, keys, counter (not the stats)
+// periods / ranges are uploaded when `upload` is set (first chunk of a batched search), else re-used.
+int run_periodic(PeriodicPlan &pl, const float2 *stats_dev, const double *periods_host, const int32_t *dur_lo_host,
+                 const int32_t *dur_hi_host, bool upload, cetra_peak *peaks_dev, void *workspace_dev,
+                 cudaStream_t st);
+int run_grids_to_stats(const float *depth_dev, const float *var_dev, int32_t n_rows, int64_t n_t0,
+                       float2 *stats_dev, cudaStream_t st);
+
+}  // namespace cetra

@@ -1,0 +1,347 @@
+"""GPU parity: the CUDA path (through the C ABI) against the FP64 oracle on the same seeded inputs.
+
+Run on the B200 box:  python -m pytest tests -m gpu -x -q
+"""
+import os
+
+import numpy as np
+import pytest
+
+from parity_util import REL, assert_linear_parity, assert_periodic_parity, period_subset
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "the -m gpu tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def cetra():
+    import paper_2503_20875_b200 as c
+    c.load_library()          # raises if the CUDA library is missing: no fallback
+    return c
+
+
+_PROBLEMS = {}
+
+
+def _problem(cfg):
+    from cetra_synth import make_config
+    if cfg not in _PROBLEMS:
+        _PROBLEMS[cfg] = make_config(cfg)
+    return _PROBLEMS[cfg]
+
+
+_ORACLE_LINEAR = {}
+
+
+def _oracle_linear(oracle_mod, cfg):
+    if cfg not in _ORACLE_LINEAR:
+        p = _problem(cfg)
+        _ORACLE_LINEAR[cfg] = oracle_mod.linear_search(p.times, p.flux, p.flux_err, p.durations, p.t0_start,
+                                                       p.t0_stride, p.n_t0, p.template)
+    return _ORACLE_LINEAR[cfg]
+
+
+def _dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _gpu_linear(torch, cetra, p, **kw):
+    return cetra.cetra_linear_search(p.times, _dev(torch, p.flux), _dev(torch, p.flux_err), p.durations, p.t0_start,
+                                     p.t0_stride, p.n_t0, p.template, **kw)
+
+
+# ------------------------------------------------------------------------------------------ linear
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_linear_search_full_grid(cfg, torch_cuda, cetra, oracle_mod):
+    """Every (t0, duration) cell of configs 1-3 (several tiles, ragged tail, the data gap, q = 6 for cfg 3)."""
+    p = _problem(cfg)
+    g = _gpu_linear(torch_cuda, cetra, p)
+    o = _oracle_linear(oracle_mod, cfg)
+    worst = assert_linear_parity(g.depth.cpu().numpy(), g.depth_var.cpu().numpy(), g.dlogL.cpu().numpy(),
+                                 o.depth, o.depth_var, o.dlogL, what=f"cfg{cfg}")
+    print(f"cfg{cfg} linear worst relative errors: {worst}")
+
+
+def test_linear_search_config4_sampled_windows(torch_cuda, cetra, oracle_mod):
+    """Config 4 at full size on the GPU; the oracle computes seeded windows of t0 cells one sub-grid at a time."""
+    p = _problem(4)
+    g = _gpu_linear(torch_cuda, cetra, p)
+    depth, var, dl = (a.cpu().numpy() for a in (g.depth, g.depth_var, g.dlogL))
+    rng = np.random.default_rng(44)
+    starts = [0, p.n_t0 - 600] + sorted(rng.integers(0, p.n_t0 - 600, size=6).tolist())
+    # one window sits on the first data gap (t = 13.2 d)
+    starts.append(int(13.2 / p.t0_stride) - 300)
+    for s in starts:
+        o = oracle_mod.linear_search(p.times, p.flux, p.flux_err, p.durations, p.t0_start + s * p.t0_stride,
+                                     p.t0_stride, 600, p.template)
+        sl = slice(s, s + 600)
+        assert_linear_parity(depth[:, sl], var[:, sl], dl[:, sl], o.depth, o.depth_var, o.dlogL,
+                             what=f"cfg4 window {s}")
+
+
+def test_linear_search_stats_are_the_sufficient_statistics(torch_cuda, cetra):
+    """stats = (S_wmm, S_wmf): depth = S_wmf/S_wmm, var = 1/S_wmm bit for bit; zero in null cells and padding."""
+    p = _problem(2)
+    g = _gpu_linear(torch_cuda, cetra, p, want_stats=True)
+    st = g.stats[0].cpu().numpy()
+    a, b = st[..., 0], st[..., 1]
+    assert np.all(st[:, p.n_t0:, :] == 0.0)
+    depth, var = g.depth.cpu().numpy(), g.depth_var.cpu().numpy()
+    null = np.isnan(depth)
+    assert null.any(), "cfg 2 has a 1 d gap: the shortest durations must have null cells"
+    assert np.all(a[:, :p.n_t0][null] == 0.0) and np.all(b[:, :p.n_t0][null] == 0.0)
+    ok = ~null
+    with np.errstate(divide="ignore", invalid="ignore"):
+        assert np.array_equal((b[:, :p.n_t0] / a[:, :p.n_t0])[ok], depth[ok])
+        assert np.array_equal((np.float32(1.0) / a[:, :p.n_t0])[ok], var[ok])
+
+
+def test_linear_search_edge_geometry(torch_cuda, cetra, oracle_mod):
+    """t0 grid that starts before the data and ends after it (R9 clipping), a stride of 3 samples with an
+    offset start, float64 input with NaN/inf/negative-error nulls, a duration shorter than the cadence,
+    a tiny n_t0 and the maximum number of durations."""
+    rng = np.random.default_rng(7)
+    n, c = 3001, 0.004
+    times = 5.0 + np.arange(n) * c
+    err = 1e-3 * (0.5 + rng.random(n))
+    flux = 1.0 + rng.standard_normal(n) * err
+    flux[100:140] = np.nan
+    err[900:960] = np.inf
+    err[1500] = -1.0
+    err[1501] = 0.0
+    flux[2000:2400] = np.nan                 # longer than most trial durations: null cells
+    from cetra_synth import tabulate_template
+    tpl = tabulate_template(257)
+    cases = [
+        dict(t0_start=times[0] - 50 * c, stride=c, n_t0=n + 120, durations=np.geomspace(0.5 * c, 300 * c, 9)),
+        dict(t0_start=times[0] + 7 * c, stride=3 * c, n_t0=977, durations=np.geomspace(2.2 * c, 111 * c, 5)),
+        dict(t0_start=times[0], stride=c, n_t0=5, durations=np.array([10 * c])),
+        dict(t0_start=times[0], stride=2 * c, n_t0=1500, durations=np.geomspace(1.5 * c, 700.3 * c, 128)),
+    ]
+    for dt in (np.float64, np.float32):
+        fl, er = flux.astype(dt), err.astype(dt)
+        for cs in cases:
+            g = cetra.cetra_linear_search(times, _dev(torch_cuda, fl), _dev(torch_cuda, er), cs["durations"],
+                                          cs["t0_start"], cs["stride"], cs["n_t0"], tpl)
+            o = oracle_mod.linear_search(times, fl, er, cs["durations"], cs["t0_start"], cs["stride"], cs["n_t0"],
+                                         tpl)
+            assert np.isnan(o.depth).any()
+            assert_linear_parity(g.depth.cpu().numpy(), g.depth_var.cpu().numpy(), g.dlogL.cpu().numpy(),
+                                 o.depth, o.depth_var, o.dlogL, what=f"edge {dt.__name__} n_t0={cs['n_t0']}")
+
+
+# ---------------------------------------------------------------------------------------- periodic
+def _oracle_periodic_inputs(oracle_mod, cfg):
+    """Oracle linear grids rounded to the float32 the GPU entry point takes, promoted back to float64."""
+    o = _oracle_linear(oracle_mod, cfg)
+    d32, v32, l32 = (a.astype(np.float32) for a in (o.depth, o.depth_var, o.dlogL))
+    grids = oracle_mod.LinearGrids(d32.astype(np.float64), v32.astype(np.float64), l32.astype(np.float64))
+    return (d32, v32, l32), grids
+
+
+def _check_periodic(torch, cetra, oracle_mod, p, grids32, grids64, sel, what, must_match=()):
+    periods = p.periods[sel]
+    peaks = cetra.cetra_periodic_search(*(_dev(torch, a) for a in grids32), p.t0_start, p.t0_stride, p.durations,
+                                        periods)
+    pk = cetra.peaks_to_numpy(peaks)[0]
+    orc = oracle_mod.periodic_search(grids64, p.t0_start, p.t0_stride, p.durations, periods)
+
+    def cell(k, j, ph):
+        return oracle_mod.periodic_cell(grids64, p.t0_stride, periods[k], j, ph)
+
+    res = assert_periodic_parity(pk, orc, cell, what=what, must_match=must_match)
+    t0_ref = p.t0_start + pk["i_t0"].astype(np.float64) * p.t0_stride
+    ok = pk["i_t0"] >= 0
+    assert np.allclose(pk["t0"][ok], t0_ref[ok], rtol=2e-7, atol=0)
+    return pk, orc, res
+
+
+def test_periodic_search_config1_all_periods(torch_cuda, cetra, oracle_mod):
+    p = _problem(1)
+    g32, g64 = _oracle_periodic_inputs(oracle_mod, 1)
+    pk, orc, res = _check_periodic(torch_cuda, cetra, oracle_mod, p, g32, g64, np.arange(p.periods.shape[0]), "cfg1")
+    print("cfg1 periodic:", res)
+
+
+@pytest.mark.parametrize("cfg,n_random", [(2, 700), (3, 500)])
+def test_periodic_search_sampled_periods(cfg, n_random, torch_cuda, cetra, oracle_mod):
+    """Configs 2-3: a seeded subset of the 20 000 trial periods plus windows around the injected period and
+    its aliases (the oracle needs ~1e6 gathers per period).  The full-K GPU run must reproduce the subset
+    run bit for bit (periods are independent), which extends the check to the bench launch configuration."""
+    p = _problem(cfg)
+    g32, g64 = _oracle_periodic_inputs(oracle_mod, cfg)
+    inj = [i["period"] for i in p.injections]
+    sel = period_subset(p.periods, inj, n_random, seed=100 + cfg)
+    k_inj = int(np.argmin(np.abs(p.periods - inj[0])))
+    must = [int(np.nonzero(sel == k_inj)[0][0])]
+    pk, orc, res = _check_periodic(torch_cuda, cetra, oracle_mod, p, g32, g64, sel, f"cfg{cfg}", must_match=must)
+    print(f"cfg{cfg} periodic:", res)
+    # injected signal: the best period of the subset is the injected one, with identical indices
+    kb_g, kb_o = int(np.nanargmax(pk["lr"])), int(np.nanargmax(orc.lr))
+    assert kb_g == kb_o
+    assert abs(p.periods[sel][kb_g] - inj[0]) <= 0.01 * inj[0]
+    assert pk["j_dur"][kb_g] == orc.j_dur[kb_o] and pk["i_t0"][kb_g] == orc.i_t0[kb_o]
+    full = cetra.peaks_to_numpy(cetra.cetra_periodic_search(*(_dev(torch_cuda, a) for a in g32), p.t0_start,
+                                                             p.t0_stride, p.durations, p.periods))[0]
+    assert np.array_equal(full[sel].view(np.uint8), pk.view(np.uint8))
+    # cfg 2 has exactly one excluded (period, duration) pair: D = 12 h = P_min (R12)
+    if cfg == 2:
+        assert np.all(full["j_dur"] < p.durations.shape[0])
+
+
+def test_periodic_search_duration_ranges_and_empty_periods(torch_cuda, cetra, oracle_mod):
+    """Per-period duration ranges, periods shorter than every duration (no candidate -> NaN
+    record, indices -1) and periods longer than the baseline (a single epoch)."""
+    p = _problem(1)
+    g32, g64 = _oracle_periodic_inputs(oracle_mod, 1)
+    periods = np.concatenate([p.periods[::7], [0.02, 0.0201, 1.2, 3.0, 50.0]])
+    K, J = periods.shape[0], p.durations.shape[0]
+    rng = np.random.default_rng(9)
+    lo = rng.integers(0, J, size=K).astype(np.int32)
+    hi = np.minimum(J, lo + rng.integers(0, 4, size=K)).astype(np.int32)      # some ranges are empty
+    peaks = cetra.cetra_periodic_search(*(_dev(torch_cuda, a) for a in g32), p.t0_start, p.t0_stride, p.durations,
+                                        periods, dur_lo=lo, dur_hi=hi)
+    pk = cetra.peaks_to_numpy(peaks)[0]
+    orc = oracle_mod.periodic_search(g64, p.t0_start, p.t0_stride, p.durations, periods, lo, hi)
+    assert np.isnan(orc.lr).any() and (~np.isnan(orc.lr)).any()
+
+    def cell(k, j, ph):
+        return oracle_mod.periodic_cell(g64, p.t0_stride, periods[k], j, ph)
+
+    assert_periodic_parity(pk, orc, cell, what="ranges")
+    ok = pk["j_dur"] >= 0
+    assert np.all(pk["j_dur"][ok] >= lo[ok]) and np.all(pk["j_dur"][ok] < hi[ok])
+
+
+# ------------------------------------------------------------------------- whole path, end to end
+def _gpu_pipeline(torch, cetra, p, periods):
+    """Linear search -> sufficient statistics -> periodic search, all on the device (the bench's path)."""
+    flux, err = _dev(torch, p.flux), _dev(torch, p.flux_err)
+    if flux.dim() == 1:
+        flux, err = flux[None], err[None]
+    peaks = cetra.cetra_search_batched(p.times, flux, err, p.durations, p.t0_start, p.t0_stride, p.n_t0, p.template,
+                                       periods)
+    return cetra.peaks_to_numpy(peaks)
+
+
+@pytest.mark.parametrize("cfg,n_random", [(1, 200), (2, 300), (3, 200)])
+def test_whole_path_against_oracle(cfg, n_random, torch_cuda, cetra, oracle_mod):
+    """FP32 linear search feeding the FP32 periodic search vs the FP64 oracle end to end; the injected
+    signal must come out at the identical (period, t0, duration) indices (north_star)."""
+    p = _problem(cfg)
+    inj = [i["period"] for i in p.injections if i["period"] is not None]
+    sel = period_subset(p.periods, inj, n_random, seed=200 + cfg)
+    periods = p.periods[sel]
+    pk = _gpu_pipeline(torch_cuda, cetra, p, periods)[0]
+    o = _oracle_linear(oracle_mod, cfg)
+    orc = oracle_mod.periodic_search(o, p.t0_start, p.t0_stride, p.durations, periods)
+
+    def cell(k, j, ph):
+        return oracle_mod.periodic_cell(o, p.t0_stride, periods[k], j, ph)
+
+    must = []
+    if inj:
+        k_inj = int(np.argmin(np.abs(p.periods - inj[0])))
+        must = [int(np.nonzero(sel == k_inj)[0][0])]
+    res = assert_periodic_parity(pk, orc, cell, what=f"cfg{cfg} end-to-end", must_match=must)
+    print(f"cfg{cfg} end-to-end:", res)
+    kb_g, kb_o = int(np.nanargmax(pk["lr"])), int(np.nanargmax(orc.lr))
+    assert kb_g == kb_o and pk["j_dur"][kb_g] == orc.j_dur[kb_o] and pk["i_t0"][kb_g] == orc.i_t0[kb_o]
+    if inj:
+        i0 = p.injections[0]
+        assert abs(periods[kb_g] - i0["period"]) <= 0.01 * i0["period"]
+        # recovered epoch and duration are the injected ones to within a grid step / one duration bin
+        t0_rec = p.t0_start + pk["i_t0"][kb_g] * p.t0_stride
+        phase_err = (t0_rec - i0["t0"] + 0.5 * i0["period"]) % i0["period"] - 0.5 * i0["period"]
+        assert abs(phase_err) <= 0.1 * i0["duration"]
+    else:
+        # cfg 1: a single transit; every period sees it once, at the injected epoch
+        i0 = p.injections[0]
+        t0_rec = p.t0_start + pk["i_t0"][kb_g] * p.t0_stride
+        assert abs(t0_rec - i0["t0"]) <= 0.1 * i0["duration"]
+
+
+def test_config4_whole_path_sampled(torch_cuda, cetra, oracle_mod):
+    """Config 4 (256 464 cells per row: the L2-gather variant of the fold kernel) on a seeded subset of its
+    200 000 periods around both injected planets; oracle linear grids in full."""
+    p = _problem(4)
+    inj = [i["period"] for i in p.injections]
+    rng = np.random.default_rng(404)
+    sel = period_subset(p.periods, inj, 0, seed=4, half_width=8)
+    sel = np.array(sorted(set(sel.tolist()) | set(rng.choice(p.periods.shape[0], 40, replace=False).tolist())))
+    periods = p.periods[sel]
+    pk = _gpu_pipeline(torch_cuda, cetra, p, periods)[0]
+    o = _oracle_linear(oracle_mod, 4)
+    orc = oracle_mod.periodic_search(o, p.t0_start, p.t0_stride, p.durations, periods)
+
+    def cell(k, j, ph):
+        return oracle_mod.periodic_cell(o, p.t0_stride, periods[k], j, ph)
+
+    res = assert_periodic_parity(pk, orc, cell, what="cfg4 end-to-end")
+    print("cfg4 end-to-end:", res)
+    # argmax within +-1 % of each injected period is the same cell on both sides
+    for i0 in p.injections:
+        near = np.abs(periods - i0["period"]) <= 0.01 * i0["period"]
+        kg = int(np.nanargmax(np.where(near, pk["lr"], -np.inf)))
+        ko = int(np.nanargmax(np.where(near, orc.lr, -np.inf)))
+        assert kg == ko and pk["j_dur"][kg] == orc.j_dur[ko] and pk["i_t0"][kg] == orc.i_t0[ko]
+
+
+# ------------------------------------------------------------------------------------------ batched
+def test_batched_equals_single_and_host_variant(torch_cuda, cetra, oracle_mod):
+    """Survey batch (config 5 recipe, 7 light curves, chunks of 3 -> ragged last chunk): the batched call,
+    the host-buffer call and one-at-a-time calls give bit-identical records; two curves are checked
+    against the oracle."""
+    from cetra_synth import make_survey_batch
+    p = make_survey_batch(n_lc=7, n_periods=600)
+    flux, err = _dev(torch_cuda, p.flux), _dev(torch_cuda, p.flux_err)
+    args = (p.durations, p.t0_start, p.t0_stride, p.n_t0, p.template, p.periods)
+    pk = cetra.peaks_to_numpy(cetra.cetra_search_batched(p.times, flux, err, *args, lc_chunk=3))
+    pk_all = cetra.peaks_to_numpy(cetra.cetra_search_batched(p.times, flux, err, *args))
+    assert np.array_equal(pk.view(np.uint8), pk_all.view(np.uint8))
+    for b in (0, 3, 6):
+        one = cetra.peaks_to_numpy(cetra.cetra_search_batched(p.times, flux[b:b + 1], err[b:b + 1], *args))
+        assert np.array_equal(one[0].view(np.uint8), pk[b].view(np.uint8))
+    host = cetra.cetra_search_batched_host(p.times, torch_cuda.from_numpy(p.flux).pin_memory(),
+                                           torch_cuda.from_numpy(p.flux_err).pin_memory(), *args, lc_chunk=3)
+    assert np.array_equal(host.view(np.uint8), pk.view(np.uint8))
+    for b in (1, 6):
+        o = oracle_mod.linear_search(p.times, p.flux[b], p.flux_err[b], p.durations, p.t0_start, p.t0_stride,
+                                     p.n_t0, p.template)
+        orc = oracle_mod.periodic_search(o, p.t0_start, p.t0_stride, p.durations, p.periods)
+
+        def cell(k, j, ph):
+            return oracle_mod.periodic_cell(o, p.t0_stride, p.periods[k], j, ph)
+
+        assert_periodic_parity(pk[b], orc, cell, what=f"batch lc {b}")
+
+
+# ------------------------------------------------------------------------------- error behaviour
+def test_status_codes_on_device(torch_cuda, cetra):
+    p = _problem(1)
+    flux, err = _dev(torch_cuda, p.flux), _dev(torch_cuda, p.flux_err)
+    bad_times = p.times.copy()
+    bad_times[500] += 0.5 * p.cadence
+    with pytest.raises(cetra.CetraError) as e:
+        cetra.cetra_linear_search(bad_times, flux, err, p.durations, p.t0_start, p.t0_stride, p.n_t0, p.template)
+    assert e.value.status == cetra.CETRA_ERR_NONUNIFORM_TIMES
+    with pytest.raises(cetra.CetraError) as e:
+        cetra.cetra_linear_search(p.times, flux, err, p.durations, p.t0_start, 1.5 * p.cadence, 100, p.template)
+    assert e.value.status == cetra.CETRA_ERR_UNSUPPORTED
+    with pytest.raises(cetra.CetraError) as e:
+        cetra.cetra_linear_search(p.times, flux, err, -p.durations, p.t0_start, p.t0_stride, p.n_t0, p.template)
+    assert e.value.status == cetra.CETRA_ERR_INVALID_ARG
+    small = torch_cuda.empty(512, dtype=torch_cuda.uint8, device="cuda")
+    with pytest.raises(cetra.CetraError) as e:
+        cetra.cetra_linear_search(p.times, flux, err, p.durations, p.t0_start, p.t0_stride, p.n_t0, p.template,
+                                  workspace=small)
+    assert e.value.status == cetra.CETRA_ERR_WORKSPACE
+    before = cetra.cetra_kernel_launch_count()
+    cetra.cetra_linear_search(p.times, flux, err, p.durations, p.t0_start, p.t0_stride, p.n_t0, p.template)
+    assert cetra.cetra_kernel_launch_count() - before == 3      # preprocess, taps, windowed sums

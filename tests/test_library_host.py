@@ -1,0 +1,131 @@
+"""CPU-side checks of the C-ABI library: it builds, loads, exports every symbol include/cetra.h declares,
+sizes its workspaces, and reports argument errors before touching the device.  No compute call here
+reaches a kernel launch (there is no GPU in the build container)."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def cetra():
+    import paper_2503_20875_b200 as c
+    c.load_library()
+    return c
+
+
+def _has_cuda():
+    import torch
+    return torch.cuda.is_available()
+
+
+def test_library_exports_every_declared_symbol(cetra):
+    header = open(os.path.join(ROOT, "include", "cetra.h")).read()
+    declared = set(re.findall(r"\b(cetra_[a-z0-9_]+)\s*\(", header))
+    assert declared == set(cetra.EXPORTED_SYMBOLS)
+    lib = cetra.load_library()
+    for name in declared:
+        assert getattr(lib, name) is not None
+
+
+def test_product_does_not_import_the_oracle():
+    """The oracle is test infrastructure: nothing under the package may import or load it."""
+    pkg = os.path.join(ROOT, "paper_2503_20875_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b|libcetra_oracle|cetra_oracle\.c|oracle/",
+                                     text, flags=re.M), f"{f} reaches into oracle/"
+
+
+def test_status_strings_and_pitch(cetra):
+    assert cetra.status_string(0) == "ok"
+    for s in (-1, -2, -3, -4, -5):
+        assert cetra.status_string(s) not in ("ok", "unknown status")
+    assert cetra.status_string(-99) == "unknown status"
+    for n_t0 in (1, 31, 32, 1000, 19728, 256464):
+        pitch = cetra.cetra_stats_pitch(n_t0)
+        assert pitch % 32 == 0 and pitch >= n_t0 + 128
+
+
+def test_workspace_sizes_scale_with_the_problem(cetra):
+    from cetra_synth import make_config
+    p = make_config(2, n_periods=100)
+    one = cetra.cetra_linear_workspace_bytes(p.times, 1, p.durations, p.t0_start, p.t0_stride, p.n_t0, 1024)
+    four = cetra.cetra_linear_workspace_bytes(p.times, 4, p.durations, p.t0_start, p.t0_stride, p.n_t0, 1024)
+    assert 0 < one < four
+    # (w f, w) per sample and light curve dominates: 8 B x N
+    assert four - one >= 3 * 8 * p.n
+    per = cetra.cetra_periodic_workspace_bytes(1, 30, p.t0_start, p.t0_stride, p.n_t0, 20000)
+    assert per >= 8 * 30 * cetra.cetra_stats_pitch(p.n_t0) + 8 * 20000 + 8 * 20000
+    b = cetra.cetra_search_batched_workspace_bytes(p.times, 1000, 0, p.durations, p.t0_start, p.t0_stride, p.n_t0,
+                                                   1024, 20000)
+    b8 = cetra.cetra_search_batched_workspace_bytes(p.times, 1000, 8, p.durations, p.t0_start, p.t0_stride, p.n_t0,
+                                                    1024, 20000)
+    assert 0 < b8 < b < 200 << 20          # the default chunk keeps the resident grids near half of L2
+    # invalid problems have no workspace size
+    bad = p.times.copy()
+    bad[10] += 0.4 * p.cadence
+    assert cetra.cetra_linear_workspace_bytes(bad, 1, p.durations, p.t0_start, p.t0_stride, p.n_t0, 1024) == 0
+
+
+def _call_linear(cetra, times, durations, t0_start, stride, n_t0, n_tpl=64, flux=0x1000, ws=0x10000, ws_bytes=1 << 30,
+                 dtype=0, n_lc=1):
+    lib = cetra.load_library()
+    from paper_2503_20875_b200.binding import cetra_t0_grid
+    times = np.ascontiguousarray(times, dtype=np.float64)
+    durations = np.ascontiguousarray(durations, dtype=np.float64)
+    tpl = np.ones(n_tpl, dtype=np.float32)
+    dp = ctypes.POINTER(ctypes.c_double)
+    return lib.cetra_linear_search(times.ctypes.data_as(dp), flux, flux, dtype, times.shape[0], n_lc,
+                                   durations.ctypes.data_as(dp), durations.shape[0],
+                                   cetra_t0_grid(t0_start, stride, n_t0), tpl.ctypes.data, n_tpl, None, None, None,
+                                   None, ws, ws_bytes, None)
+
+
+def test_argument_errors_are_reported_without_a_device(cetra):
+    """Validation happens before any device work, so these statuses are the same on a CPU-only host."""
+    c = 0.01
+    times = np.arange(500) * c
+    dur = np.array([0.05, 0.1])
+    ok_args = (times, dur, 0.0, c, 500)
+    assert _call_linear(cetra, *ok_args, flux=None) == cetra.CETRA_ERR_INVALID_ARG
+    assert _call_linear(cetra, *ok_args, dtype=7) == cetra.CETRA_ERR_INVALID_ARG
+    assert _call_linear(cetra, times, -dur, 0.0, c, 500) == cetra.CETRA_ERR_INVALID_ARG
+    assert _call_linear(cetra, times, dur, 0.0, c, 0) == cetra.CETRA_ERR_INVALID_ARG
+    assert _call_linear(cetra, times, dur, 0.0, -c, 500) == cetra.CETRA_ERR_INVALID_ARG
+    assert _call_linear(cetra, times, np.full(129, 0.05), 0.0, c, 500) == cetra.CETRA_ERR_UNSUPPORTED
+    assert _call_linear(cetra, times, dur, 0.0, 1.5 * c, 100) == cetra.CETRA_ERR_UNSUPPORTED
+    assert _call_linear(cetra, times, dur, 0.25 * c, c, 100) == cetra.CETRA_ERR_UNSUPPORTED
+    jitter = times.copy()
+    jitter[123] += 0.01 * c
+    assert _call_linear(cetra, jitter, dur, 0.0, c, 500) == cetra.CETRA_ERR_NONUNIFORM_TIMES
+    assert _call_linear(cetra, *ok_args, ws=None) == cetra.CETRA_ERR_WORKSPACE
+    assert _call_linear(cetra, *ok_args, ws=0x10008) == cetra.CETRA_ERR_WORKSPACE      # misaligned
+    assert _call_linear(cetra, *ok_args, ws_bytes=1024) == cetra.CETRA_ERR_WORKSPACE
+
+
+def test_compute_fails_loudly_without_a_device(cetra):
+    """No CPU fallback: with valid arguments and no GPU the entry point returns CETRA_ERR_CUDA, and the
+    Python binding refuses to run."""
+    if _has_cuda():
+        pytest.skip("a CUDA device is present")
+    c = 0.01
+    times = np.arange(500) * c
+    assert _call_linear(cetra, times, np.array([0.05]), 0.0, c, 500) == cetra.CETRA_ERR_CUDA
+    import torch
+    with pytest.raises((RuntimeError, TypeError)):
+        cetra.cetra_linear_search(times, torch.ones(500), torch.ones(500), np.array([0.05]), 0.0, c, 500,
+                                  np.ones(16, np.float32))
+
+
+def test_peak_record_layout(cetra):
+    from paper_2503_20875_b200.binding import cetra_peak
+    assert ctypes.sizeof(cetra_peak) == 32 == cetra.PEAK_DTYPE.itemsize
+    for name, _ in cetra_peak._fields_:
+        assert getattr(cetra_peak, name).offset == cetra.PEAK_DTYPE.fields[name][1]
