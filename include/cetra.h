@@ -180,6 +180,17 @@ int cetra_search_batched_host(const double *times_host, const void *flux_host, c
 /* Number of kernel launches the library has enqueued since the process started (diagnostic). */
 int64_t cetra_kernel_launch_count(void);
 
+/* Diagnostics for bench.py's roofline line.  While enabled, the library brackets every launch of its two
+ * hot kernels (the windowed-sum linear-search kernel and the fold-gather-argmax periodic-search kernel)
+ * with a pair of CUDA events recorded on the launching stream; nothing is synchronised at launch time.
+ * The events are the only objects the library ever creates; cetra_profile_enable(0) destroys them.
+ * cetra_profile_read waits for the recorded events, returns the summed device time (milliseconds) and the
+ * number of launches of each kernel since the last reset, and resets the counters if `reset` is non-zero.
+ * Any output pointer may be NULL.  Not thread-safe. */
+int cetra_profile_enable(int32_t enable);
+int cetra_profile_read(double *linear_ms, int64_t *linear_launches, double *fold_ms, int64_t *fold_launches,
+                       int32_t reset);
+
 #ifdef __cplusplus
 }
 #endif

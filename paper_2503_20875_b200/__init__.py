@@ -22,6 +22,8 @@ from .binding import (  # noqa: F401
     cetra_linear_search,
     cetra_linear_workspace_bytes,
     cetra_periodic_search,
+    cetra_profile_enable,
+    cetra_profile_read,
     cetra_periodic_search_stats,
     cetra_periodic_workspace_bytes,
     cetra_search_batched,

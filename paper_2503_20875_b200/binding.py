@@ -32,6 +32,7 @@ EXPORTED_SYMBOLS = (
     "cetra_periodic_workspace_bytes", "cetra_periodic_search", "cetra_periodic_search_stats",
     "cetra_search_batched_workspace_bytes", "cetra_search_batched",
     "cetra_search_batched_host_workspace_bytes", "cetra_search_batched_host",
+    "cetra_profile_enable", "cetra_profile_read",
 )
 
 
@@ -99,6 +100,10 @@ def load_library() -> ctypes.CDLL:
     lib.cetra_search_batched_host.restype = ctypes.c_int
     lib.cetra_search_batched_host.argtypes = [dp, vp, vp, ctypes.c_int, i64, i32, i32, dp, i32, cetra_t0_grid, fp,
                                               i32, dp, i32, ip, ip, vp, vp, sz, vp]
+    lib.cetra_profile_enable.restype = ctypes.c_int
+    lib.cetra_profile_enable.argtypes = [i32]
+    lib.cetra_profile_read.restype = ctypes.c_int
+    lib.cetra_profile_read.argtypes = [dp, ctypes.POINTER(i64), dp, ctypes.POINTER(i64), i32]
     _lib = lib
     return lib
 
@@ -187,6 +192,19 @@ def cetra_stats_pitch(n_t0: int) -> int:
 
 def cetra_kernel_launch_count() -> int:
     return int(load_library().cetra_kernel_launch_count())
+
+
+def cetra_profile_enable(enable: bool) -> None:
+    _check(load_library().cetra_profile_enable(1 if enable else 0), "cetra_profile_enable")
+
+
+def cetra_profile_read(reset: bool = True):
+    """{'linear_ms', 'linear_launches', 'fold_ms', 'fold_launches'} since the last reset (waits for the events)."""
+    lm, fm = ctypes.c_double(), ctypes.c_double()
+    ll, fl = ctypes.c_int64(), ctypes.c_int64()
+    _check(load_library().cetra_profile_read(ctypes.byref(lm), ctypes.byref(ll), ctypes.byref(fm), ctypes.byref(fl),
+                                             1 if reset else 0), "cetra_profile_read")
+    return dict(linear_ms=lm.value, linear_launches=ll.value, fold_ms=fm.value, fold_launches=fl.value)
 
 
 def cetra_linear_workspace_bytes(times, n_lc: int, durations, t0_start, t0_stride, n_t0, n_template: int) -> int:

@@ -5,6 +5,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <vector>
 
 #include "linear_search.cuh"
 #include "periodic_search.cuh"
@@ -12,6 +13,41 @@
 namespace cetra {
 
 std::atomic<int64_t> g_launch_count{0};
+
+// ---- optional profiling events (diagnostics only) ----
+struct ProfileState {
+    bool on = false;
+    std::vector<cudaEvent_t> begin[2], end[2];
+    double ms[2] = {0.0, 0.0};
+    int64_t launches[2] = {0, 0};
+};
+static ProfileState g_prof;
+
+void profile_mark(ProfiledKernel which, bool begin, cudaStream_t st) {
+    if (!g_prof.on) return;
+    cudaEvent_t ev;
+    if (cudaEventCreate(&ev) != cudaSuccess) return;
+    cudaEventRecord(ev, st);
+    (begin ? g_prof.begin[which] : g_prof.end[which]).push_back(ev);
+}
+
+static void profile_drain() {
+    for (int w = 0; w < 2; ++w) {
+        const size_t n = std::min(g_prof.begin[w].size(), g_prof.end[w].size());
+        for (size_t i = 0; i < n; ++i) {
+            float ms = 0.f;
+            if (cudaEventSynchronize(g_prof.end[w][i]) == cudaSuccess &&
+                cudaEventElapsedTime(&ms, g_prof.begin[w][i], g_prof.end[w][i]) == cudaSuccess) {
+                g_prof.ms[w] += ms;
+                g_prof.launches[w] += 1;
+            }
+        }
+        for (cudaEvent_t e : g_prof.begin[w]) cudaEventDestroy(e);
+        for (cudaEvent_t e : g_prof.end[w]) cudaEventDestroy(e);
+        g_prof.begin[w].clear();
+        g_prof.end[w].clear();
+    }
+}
 
 // DESIGN.md R1/R9: the samples are a regular grid; the t0 grid sits on it with a whole-sample stride.
 int derive_geometry(const double *times_host, int64_t n, cetra_t0_grid grid, Geometry *g) {
@@ -104,6 +140,28 @@ int cetra_device_info(int32_t *n_sm, int32_t *smem_per_block_optin) {
 int64_t cetra_stats_pitch(int64_t n_t0) { return round_up64(n_t0 + kStatsPad, 32); }
 
 int64_t cetra_kernel_launch_count(void) { return g_launch_count.load(); }
+
+int cetra_profile_enable(int32_t enable) {
+    profile_drain();
+    g_prof.on = enable != 0;
+    g_prof.ms[0] = g_prof.ms[1] = 0.0;
+    g_prof.launches[0] = g_prof.launches[1] = 0;
+    return CETRA_OK;
+}
+
+int cetra_profile_read(double *linear_ms, int64_t *linear_launches, double *fold_ms, int64_t *fold_launches,
+                       int32_t reset) {
+    profile_drain();
+    if (linear_ms) *linear_ms = g_prof.ms[kProfLinear];
+    if (linear_launches) *linear_launches = g_prof.launches[kProfLinear];
+    if (fold_ms) *fold_ms = g_prof.ms[kProfFold];
+    if (fold_launches) *fold_launches = g_prof.launches[kProfFold];
+    if (reset) {
+        g_prof.ms[0] = g_prof.ms[1] = 0.0;
+        g_prof.launches[0] = g_prof.launches[1] = 0;
+    }
+    return cudaGetLastError() == cudaSuccess ? CETRA_OK : CETRA_ERR_CUDA;
+}
 
 // ------------------------------------------------------------------------------------------ linear
 size_t cetra_linear_workspace_bytes(const double *times_host, int64_t n, int32_t n_lc, const double *durations_host,

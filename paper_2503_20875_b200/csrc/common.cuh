@@ -24,6 +24,10 @@ extern std::atomic<int64_t> g_launch_count;
         if (cudaPeekAtLastError() != cudaSuccess) return CETRA_ERR_CUDA; \
     } while (0)
 
+// Optional event bracketing of the two hot kernels (cetra_profile_enable / cetra_profile_read).
+enum ProfiledKernel { kProfLinear = 0, kProfFold = 1 };
+void profile_mark(ProfiledKernel which, bool begin, cudaStream_t st);
+
 constexpr int kStatsPad = 128;          // zero cells after the last t0 cell of every stats row
 constexpr size_t kAlign = 256;          // workspace carve-up alignment
 

@@ -316,11 +316,15 @@ int run_linear(LinearPlan &pl, const void *flux_dev, const void *flux_err_dev, c
     }
     const long long blocks = static_cast<long long>(P.tiles_per_row) * P.n_dur * n_lc;
     constexpr int R = kLinearR;
+    profile_mark(kProfLinear, true, st);
+    int rc;
     switch (pl.warps) {
-        case 4: return launch_linear<R, 4>(pl, P, blocks, st);
-        case 2: return launch_linear<R, 2>(pl, P, blocks, st);
-        default: return launch_linear<R, 1>(pl, P, blocks, st);
+        case 4: rc = launch_linear<R, 4>(pl, P, blocks, st); break;
+        case 2: rc = launch_linear<R, 2>(pl, P, blocks, st); break;
+        default: rc = launch_linear<R, 1>(pl, P, blocks, st); break;
     }
+    profile_mark(kProfLinear, false, st);
+    return rc;
 }
 
 }  // namespace cetra

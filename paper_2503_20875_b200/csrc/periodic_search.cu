@@ -297,6 +297,7 @@ int run_periodic(PeriodicPlan &pl, const float2 *stats_dev, const double *period
     P.keys = keys;
     P.counter = reinterpret_cast<unsigned int *>(keys + n_keys);
     CETRA_CUDA_TRY(cudaMemsetAsync(keys, 0, sizeof(unsigned long long) * (n_keys + 32), st));
+    profile_mark(kProfFold, true, st);
     if (pl.row_in_smem) {
         auto k = fold_argmax_kernel<true>;
         CETRA_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes));
@@ -304,6 +305,7 @@ int run_periodic(PeriodicPlan &pl, const float2 *stats_dev, const double *period
     } else {
         fold_argmax_kernel<false><<<pl.grid, kFoldThreads, pl.smem_bytes, st>>>(P);
     }
+    profile_mark(kProfFold, false, st);
     CETRA_LAUNCH_CHECK();
     {
         const long long total = static_cast<long long>(P.n_lc) * P.n_per;
