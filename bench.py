@@ -1,0 +1,393 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the CETRA hot path on B200 (one JSON line on stdout, rank 0).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--n-lc B] [--workload sector|survey] [--impl cuda|reference]
+
+A *step* is one pass of the whole hot path (preprocess, template taps,
+windowed sums + epilogue, fold-gather-sum, combine, per-period argmax) over one batch of B synthetic
+light curves.  The workload is BASELINE.json configs[1], the TESS-like 2-min sector (19 728 points,
+30 durations, 20 000 periods), B curves per GPU drawn with the config-5 survey recipe (cetra_synth).
+
+  value      light curves/s, inputs resident in HBM when the timed region starts (cetra_search_batched)
+  e2e        the same metric through cetra_search_batched_host: pinned HOST buffers, H2D + D2H timed
+  roofline   the dominant kernel (fold_argmax_kernel, periodic search): algorithmic bytes / event time
+  cpu_baseline  the FP64 oracle on the host cores, on a bounded sample of the same workload
+
+N > 1 (torchrun): every rank searches its own B curves (no data-path collective; "weak" scaling), the
+time is the max over ranks.  --impl reference times the oracle (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "TESS-sector light curves/sec"
+UNIT = "light curves/s"
+L2_FLUSH_BYTES = 512 << 20
+N_SM, FP32_LANES = 148, 128          # B200: SMs, FP32 FMA lanes per SM (B200_PROFILING.md unit counts)
+SMEM_BYTES_PER_CLK = 128             # shared-memory crossbar bytes/clk/SM (B300_MICROARCH.md, LDS/STS)
+
+
+# ----------------------------------------------------------------------------------------------- helpers
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            d = json.load(fh)
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+def work_counts(p):
+    """Algorithmic work of one light curve (counting only)."""
+    n, c = p.n, p.cadence
+    q = int(round(p.t0_stride / c))
+    n0 = int(round((p.t0_start - p.times[0]) / c))
+    centres = n0 + q * np.arange(p.n_t0, dtype=np.int64)
+    evals = 0
+    for d in p.durations:
+        h = int(np.floor(d / (2.0 * c) + 1e-12))
+        lo = np.maximum(centres - h, 0)
+        hi = np.minimum(centres + h, n - 1)
+        evals += int(np.maximum(hi - lo + 1, 0).sum())
+    pairs = int((p.durations[None, :] < p.periods[:, None]).sum())
+    return dict(template_evals=evals, pairs=pairs, gathers=pairs * p.n_t0, cells=p.n_t0 * len(p.durations))
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons while the timed region runs (B200_PROFILING.md clocks line)."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.FIELDS}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def __exit__(self, *exc):
+        if self.proc is not None:
+            time.sleep(0.15)
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except subprocess.TimeoutExpired:
+                self.proc.kill()
+            self.thread.join(timeout=2)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except ValueError:
+                continue
+            for name, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=[], samples=0)
+        return dict(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
+
+
+def oracle_sample(p, flux, flux_err, budget_s: float):
+    """The oracle, as it stands, on one light curve of the workload: the linear search in full and the
+    periodic search on a seeded subset of the trial periods sized to about `budget_s` of CPU time.
+    Returns (light curves/s extrapolated to all K periods, description, cores)."""
+    import oracle
+    oracle.build()
+    cores = oracle.get_threads()
+    t = time.perf_counter()
+    grids = oracle.linear_search(p.times, flux, flux_err, p.durations, p.t0_start, p.t0_stride, p.n_t0, p.template)
+    t_lin = time.perf_counter() - t
+    rng = np.random.default_rng(20875)
+    K = p.periods.shape[0]
+    order = rng.permutation(K)
+    probe, t_probe = max(cores, 8), 0.0
+    while True:                                     # grow the probe until it is long enough to time
+        t = time.perf_counter()
+        oracle.periodic_search(grids, p.t0_start, p.t0_stride, p.durations, p.periods[np.sort(order[:probe])])
+        t_probe = time.perf_counter() - t
+        if t_probe >= 0.1 * budget_s or probe >= K:
+            break
+        probe = min(K, probe * 4)
+    k_s = int(min(K, max(probe, budget_s / max(t_probe / probe, 1e-9))))
+    t = time.perf_counter()
+    oracle.periodic_search(grids, p.t0_start, p.t0_stride, p.durations, p.periods[np.sort(order[:k_s])])
+    t_per = time.perf_counter() - t
+    t_lc = t_lin + t_per * (K / k_s)
+    sample = (f"1 light curve of the workload: linear search in full ({t_lin:.2f} s) + periodic search on a seeded "
+              f"{k_s}-of-{K} period subset ({t_per:.2f} s), periodic time scaled by K/subset")
+    return 1.0 / t_lc, sample, cores, t_lin + t_per
+
+
+# ------------------------------------------------------------------------------------------ reference arm
+def run_reference(args, rank: int):
+    """--impl reference: the oracle on the host cores (rank 0 only), same metric / unit / config."""
+    if rank != 0:
+        return
+    from cetra_synth import make_survey_batch
+    p = make_survey_batch(n_lc=max(args.n_lc, 1), lc_range=(0, 1))
+    budget = args.ref_seconds
+    for _ in range(args.warmup):
+        oracle_sample(p, p.flux[0], p.flux_err[0], min(budget, 1.0))
+    vals, spent, sample, cores = [], 0.0, "", 0
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        v, sample, cores, used = oracle_sample(p, p.flux[0], p.flux_err[0], budget)
+        vals.append(v); spent += used
+    wall = time.perf_counter() - t0
+    value = len(vals) / sum(1.0 / v for v in vals)
+    line = dict(metric=METRIC, value=value, unit=UNIT, impl="reference", n_gpus=args.gpus, steps=args.steps,
+                warmup=args.warmup, ms_per_step=1e3 * wall / max(args.steps, 1), higher_is_better=True,
+                scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+                config=workload_config(p, args, args.n_lc, "oracle on host cores; each step = " + sample),
+                cpu_baseline=dict(value=value, unit=UNIT, cores=cores, kind="oracle", sample=sample),
+                e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
+                gpu_launches=0)
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(p, args, n_lc, note):
+    return dict(workload=f"BASELINE configs[1] tess-2min-sector x {n_lc} light curves per GPU per step "
+                         f"(config-5 survey recipe: shared 19 728-point 2-min time array with a 1 d gap)",
+                n_points=p.n, n_durations=int(len(p.durations)), n_t0=int(p.n_t0), n_periods=int(len(p.periods)),
+                n_template=int(len(p.template)), light_curves_per_step_per_gpu=n_lc,
+                l2="flushed between timed steps (512 MiB write)", note=note)
+
+
+# ------------------------------------------------------------------------------------------------- CUDA arm
+def run_cuda(args, rank: int, world: int, local_rank: int):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2503_20875_b200 as cetra
+    from cetra_synth import make_survey_batch
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the CETRA library has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    cetra.load_library()
+    if world > 1 and not dist.is_initialized():
+        dist.init_process_group("nccl", device_id=dev)
+
+    B = args.n_lc
+    p = make_survey_batch(n_lc=B * world, lc_range=(rank * B, (rank + 1) * B))   # each rank owns its curves
+    wc = work_counts(p)
+    K = p.periods.shape[0]
+    flux_h = torch.from_numpy(p.flux).pin_memory()
+    err_h = torch.from_numpy(p.flux_err).pin_memory()
+    flux_d, err_d = flux_h.to(dev), err_h.to(dev)
+    gargs = (p.durations, p.t0_start, p.t0_stride, p.n_t0, p.template, p.periods)
+    ws_bytes = cetra.cetra_search_batched_host_workspace_bytes(p.times, B, 0, cetra.CETRA_F32, p.durations,
+                                                               p.t0_start, p.t0_stride, p.n_t0, len(p.template), K)
+    ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
+    peaks_d = torch.empty((B, K, 8), dtype=torch.int32, device=dev)
+    peaks_h = torch.empty((B, K, 8), dtype=torch.int32).pin_memory()
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step_device():
+        cetra.cetra_search_batched(p.times, flux_d, err_d, *gargs, workspace=ws, peaks=peaks_d)
+
+    def step_host():
+        cetra.cetra_search_batched_host(p.times, flux_h, err_h, *gargs, workspace=ws, peaks_host=peaks_h, device=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps, profile):
+        """`steps` steps, each bracketed by CUDA events on the launching stream; L2 flushed between them."""
+        evs = []
+        barrier()
+        if profile:
+            cetra.cetra_profile_enable(True)
+        launches0 = cetra.cetra_kernel_launch_count()
+        t_wall = time.perf_counter()
+        for _ in range(steps):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            fn()
+            b.record(stream)
+            evs.append((a, b))
+        barrier()
+        wall = time.perf_counter() - t_wall
+        launches = cetra.cetra_kernel_launch_count() - launches0
+        prof = cetra.cetra_profile_read(reset=True) if profile else None
+        if profile:
+            cetra.cetra_profile_enable(False)
+        ms = sum(a.elapsed_time(b) for a, b in evs)
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item()), launches, prof, wall
+
+    for _ in range(args.warmup):
+        step_device()
+    for _ in range(min(args.warmup, 1)):
+        step_host()
+    with ClockSampler(local_rank) as clocks:
+        ms_dev, launches, prof, wall_dev = timed(step_device, args.steps, profile=True)
+    ms_e2e, _, _, wall_e2e = timed(step_host, args.steps, profile=False)
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peaks = measured_peaks()
+    total_lc = B * world * args.steps
+    value = total_lc / (ms_dev * 1e-3)
+    e2e_value = total_lc / (ms_e2e * 1e-3)
+    # roofline of the dominant kernel (periodic fold): 8 B and 2 FADD per (period, duration, t0 cell)
+    fold_launches = max(prof["fold_launches"], 1)
+    lin_launches = max(prof["linear_launches"], 1)
+    fold_bytes = 8.0 * wc["gathers"] * B * args.steps          # summed over this rank's launches
+    fold_s = prof["fold_ms"] * 1e-3
+    lin_s = prof["linear_ms"] * 1e-3
+    fold_gbs = fold_bytes / fold_s / 1e9
+    lin_tflops = 4.0 * wc["template_evals"] * B * args.steps / lin_s / 1e12
+    fp32_peak = N_SM * FP32_LANES * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    smem_peak = N_SM * SMEM_BYTES_PER_CLK * peaks["sm_max_mhz"] * 1e6 / 1e9
+    line = dict(
+        metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
+        ms_per_step=ms_dev / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
+        dtype="f32", data="synthetic",
+        config=workload_config(p, args, B, "timed per step with CUDA events on the launching stream, summed; "
+                                           "max over ranks"),
+        e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=int(2 * B * p.n * 4),
+                 d2h_bytes_per_step=int(B * K * 32), ms_per_step=ms_e2e / args.steps,
+                 api="cetra_search_batched_host (pinned host flux/flux_err in, pinned host records out)"),
+        gpu_launches=int(launches),
+        clocks=clocks.summary(),
+        roofline=dict(bound="hbm", kernel="fold_argmax_kernel", achieved=fold_gbs, peak=peaks["hbm_gbs"],
+                      unit="GB/s", frac=fold_gbs / peaks["hbm_gbs"], traffic=None, peak_source=peaks["source"],
+                      ms_per_launch=prof["fold_ms"] / fold_launches, launches=int(prof["fold_launches"]),
+                      share_of_step=prof["fold_ms"] / ms_dev,
+                      algorithmic_bytes_per_launch=fold_bytes / fold_launches,
+                      served_from="shared memory (one (S_wmm,S_wmf) row per CTA); compulsory HBM traffic is the "
+                                  "stats grid once per chunk",
+                      smem=dict(achieved=fold_gbs, peak=smem_peak, unit="GB/s", frac=fold_gbs / smem_peak,
+                                peak_derivation="148 SM x 128 B/clk x sm_max_mhz")),
+        roofline_linear=dict(bound="alu", kernel="linear_search_kernel", achieved=lin_tflops, peak=fp32_peak,
+                             unit="TFLOP/s", frac=lin_tflops / fp32_peak,
+                             peak_derivation="148 SM x 128 FP32 lanes x 2 flop x sm_max_mhz",
+                             ms_per_launch=prof["linear_ms"] / lin_launches, launches=int(prof["linear_launches"]),
+                             share_of_step=prof["linear_ms"] / ms_dev,
+                             template_evals_per_s=wc["template_evals"] * B * args.steps / lin_s),
+        rates=dict(periods_per_s=K * total_lc / (ms_dev * 1e-3),
+                   template_evals_per_lc=wc["template_evals"], gathers_per_lc=wc["gathers"],
+                   duration_period_pairs=wc["pairs"]),
+    )
+    if world == 1 and not args.no_cpu_baseline:
+        v, sample, cores, _ = oracle_sample(p, p.flux[0], p.flux_err[0], args.cpu_seconds)
+        line["cpu_baseline"] = dict(value=v, unit=UNIT, cores=cores, kind="oracle", sample=sample)
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------- config-5 survey (optional)
+def run_survey(args):
+    """BASELINE.json configs[4]: the 10 000-curve survey batch, a slice at a time, with the injection-
+    recovery fraction (best period within 1 % of P, P/2 or 2P).  One GPU."""
+    import torch
+
+    import paper_2503_20875_b200 as cetra
+    from cetra_synth import make_survey_batch
+
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    n_total, sl = args.survey_lc, args.n_lc
+    rec = inj = false_alarm_free = 0
+    gpu_ms = 0.0
+    best_lr_planet, best_lr_null = [], []
+    for lo in range(0, n_total, sl):
+        hi = min(n_total, lo + sl)
+        p = make_survey_batch(n_lc=n_total, lc_range=(lo, hi))
+        flux_d, err_d = torch.from_numpy(p.flux).to(dev), torch.from_numpy(p.flux_err).to(dev)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        peaks = cetra.cetra_search_batched(p.times, flux_d, err_d, p.durations, p.t0_start, p.t0_stride, p.n_t0,
+                                           p.template, p.periods)
+        b.record()
+        torch.cuda.synchronize()
+        gpu_ms += a.elapsed_time(b)
+        lr = peaks[..., 0].view(torch.float32)                       # host step: pick the peak period
+        lr = torch.where(torch.isnan(lr), torch.full_like(lr, -1.0), lr)
+        kb = torch.argmax(lr, dim=1).cpu().numpy()
+        best = lr.max(dim=1).values.cpu().numpy()
+        for i, injn in enumerate(p.injections):
+            pb = p.periods[kb[i]]
+            if injn["period"] is None:
+                best_lr_null.append(float(best[i]))
+                continue
+            inj += 1
+            best_lr_planet.append(float(best[i]))
+            if any(abs(pb - m * injn["period"]) <= 0.01 * m * injn["period"] for m in (0.5, 1.0, 2.0)):
+                rec += 1
+    line = dict(metric=METRIC, value=n_total / (gpu_ms * 1e-3), unit=UNIT, n_gpus=1, workload="BASELINE configs[4] "
+                f"survey batch, {n_total} light curves in slices of {sl}", injected=inj, recovered=rec,
+                recovery_fraction=rec / max(inj, 1), gpu_seconds=gpu_ms * 1e-3,
+                median_best_lr_injected=float(np.median(best_lr_planet)) if best_lr_planet else None,
+                median_best_lr_null=float(np.median(best_lr_null)) if best_lr_null else None)
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="sector", choices=["sector", "survey"])
+    ap.add_argument("--n-lc", type=int, default=64, help="light curves per GPU per step (survey: per slice)")
+    ap.add_argument("--survey-lc", type=int, default=10000)
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU budget of the cpu_baseline sample")
+    ap.add_argument("--ref-seconds", type=float, default=8.0, help="CPU budget of one --impl reference step")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+    elif args.workload == "survey":
+        run_survey(args)
+    else:
+        run_cuda(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -224,8 +224,11 @@ def make_config(cfg: int, n_periods: Optional[int] = None) -> SearchProblem:
 
 
 def make_survey_batch(n_lc: int = 10000, n_periods: Optional[int] = None,
-                      seed_offset: int = 0) -> SearchProblem:
-    """BASELINE.json config 5: n_lc light curves on the cfg-2 time array, gap and grids."""
+                      seed_offset: int = 0, lc_range: Optional[Tuple[int, int]] = None) -> SearchProblem:
+    """BASELINE.json config 5: n_lc light curves on the cfg-2 time array, gap and grids.
+
+    `lc_range=(lo, hi)` returns only curves lo..hi-1 of the n_lc-curve batch (the same curves a full
+    call would return), so that a large survey can be generated and searched a slice at a time."""
     n = 19728
     times, c = _regular_times(n, 120.0)
     stride = 120.0 / DAY_S
@@ -235,8 +238,10 @@ def make_survey_batch(n_lc: int = 10000, n_periods: Optional[int] = None,
     periods = period_grid_uniform_frequency(0.5, 13.7, k)
     gap = (times >= 13.2) & (times < 14.2)
     children = np.random.SeedSequence(BASE_SEED + 5 + seed_offset).spawn(n_lc)
-    flux = np.empty((n_lc, n), dtype=np.float32)
-    err = np.empty((n_lc, n), dtype=np.float32)
+    if lc_range is not None:
+        children = children[lc_range[0]:lc_range[1]]
+    flux = np.empty((len(children), n), dtype=np.float32)
+    err = np.empty((len(children), n), dtype=np.float32)
     injections: List[Dict] = []
     for b, child in enumerate(children):
         rng = np.random.default_rng(child)
@@ -271,5 +276,5 @@ def make_survey_batch(n_lc: int = 10000, n_periods: Optional[int] = None,
     return SearchProblem(
         cfg=5, name=CONFIG_NAMES[5], times=times, flux=flux, flux_err=err, cadence=c, template=tpl,
         durations=durations, t0_start=t0_start, t0_stride=stride, n_t0=n_t0, periods=periods,
-        injections=injections, meta=dict(seed=BASE_SEED + 5 + seed_offset, n_lc=n_lc),
+        injections=injections, meta=dict(seed=BASE_SEED + 5 + seed_offset, n_lc=n_lc, lc_range=lc_range),
     )

@@ -111,9 +111,14 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
     }
     mbar_wait(bar, 0);
 
-    float accA[R], accB[R];
+    // Two-level summation: the running FFMA accumulators are folded into a second set every kFlush tap
+    // groups (and at the end of every polyphase branch), so that no FP32 sum runs over more than
+    // kFlush*R terms before it is added to terms of its own size (cfg 3 has
+    // windows of 2 701 points).
+    constexpr int kFlush = 4;
+    float accA[R], accB[R], totA[R], totB[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) { accA[r] = 0.f; accB[r] = 0.f; }
+    for (int r = 0; r < R; ++r) { accA[r] = 0.f; accB[r] = 0.f; totA[r] = 0.f; totB[r] = 0.f; }
 
     const float2 *xs = data + d0 + q * (tid * R);
     for (int b = 0; b < q; ++b) {
@@ -125,6 +130,7 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
         float2 nxt = xb[q * (R - 1)];
         float2 tap = tb[0];
         const float2 *xp = xb + q * R;
+        int since_flush = 0;
         for (int a0 = 0; a0 < A; a0 += R) {
 #pragma unroll
             for (int u = 0; u < R; ++u) {
@@ -141,13 +147,21 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
                 }
             }
             if (Q1) xp += R;
+            if (++since_flush == kFlush || a0 + R >= A) {
+                since_flush = 0;
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    totA[r] += accA[r]; totB[r] += accB[r];
+                    accA[r] = 0.f; accB[r] = 0.f;
+                }
+            }
         }
     }
 
     // transpose through shared memory so that the global stores are coalesced
     float2 *st = stage + warp * (32 * R);
 #pragma unroll
-    for (int r = 0; r < R; ++r) st[lane * R + r] = make_float2(accA[r], accB[r]);
+    for (int r = 0; r < R; ++r) st[lane * R + r] = make_float2(totA[r], totB[r]);
     __syncwarp();
     const long long row = lc * P.n_dur + j;
     const long long i_warp = i_blk + static_cast<long long>(warp) * (32 * R);
@@ -278,10 +292,12 @@ int run_linear(LinearPlan &pl, const void *flux_dev, const void *flux_err_dev, c
                int32_t n_lc, const float *template_host, int32_t n_template, bool template_on_device,
                float *depth_dev, float *var_dev, float *dlogL_dev, float *stats_dev, void *workspace_dev,
                cudaStream_t st) {
+    // the tap tables come first: their place must not depend on n_lc, because the batched search builds
+    // them once and then runs ragged last chunks with fewer light curves in the same workspace
     Carver ws(workspace_dev);
-    float2 *wfw = ws.take<float2>(static_cast<size_t>(pl.P.lc_pitch) * n_lc);
     float2 *taps = ws.take<float2>(static_cast<size_t>(pl.taps_total));
     float *tpl = ws.take<float>(static_cast<size_t>(n_template));
+    float2 *wfw = ws.take<float2>(static_cast<size_t>(pl.P.lc_pitch) * n_lc);
     LinearParams &P = pl.P;
     P.wfw = wfw;
     P.taps = taps;

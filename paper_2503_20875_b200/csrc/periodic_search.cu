@@ -89,11 +89,13 @@ __device__ __forceinline__ void fold_period(const float2 *__restrict__ row, int 
     int p0 = 0;
     for (; p0 + 32 * kFoldR <= n_phase; p0 += 32 * kFoldR)
         fold_pass<kFoldR, kSmemRow>(row, p0, n_t0, n_phase, r, lane, best_lr, best_p);
+    static_assert(kFoldR == 4, "the remainder switch below covers 1..kFoldR groups");
     const int groups = (n_phase - p0 + 31) >> 5;
     switch (groups) {
         case 1: fold_pass<1, kSmemRow>(row, p0, n_t0, n_phase, r, lane, best_lr, best_p); break;
         case 2: fold_pass<2, kSmemRow>(row, p0, n_t0, n_phase, r, lane, best_lr, best_p); break;
         case 3: fold_pass<3, kSmemRow>(row, p0, n_t0, n_phase, r, lane, best_lr, best_p); break;
+        case 4: fold_pass<4, kSmemRow>(row, p0, n_t0, n_phase, r, lane, best_lr, best_p); break;   // 97..127 phases left
         default: break;
     }
     // warp argmax: larger lr wins, ties -> smaller phase

@@ -124,6 +124,7 @@ def test_linear_search_edge_geometry(torch_cuda, cetra, oracle_mod):
         dict(t0_start=times[0], stride=c, n_t0=5, durations=np.array([10 * c])),
         dict(t0_start=times[0], stride=2 * c, n_t0=1500, durations=np.geomspace(1.5 * c, 700.3 * c, 128)),
     ]
+    saw_null = False
     for dt in (np.float64, np.float32):
         fl, er = flux.astype(dt), err.astype(dt)
         for cs in cases:
@@ -131,9 +132,10 @@ def test_linear_search_edge_geometry(torch_cuda, cetra, oracle_mod):
                                           cs["t0_start"], cs["stride"], cs["n_t0"], tpl)
             o = oracle_mod.linear_search(times, fl, er, cs["durations"], cs["t0_start"], cs["stride"], cs["n_t0"],
                                          tpl)
-            assert np.isnan(o.depth).any()
+            saw_null |= bool(np.isnan(o.depth).any())
             assert_linear_parity(g.depth.cpu().numpy(), g.depth_var.cpu().numpy(), g.dlogL.cpu().numpy(),
                                  o.depth, o.depth_var, o.dlogL, what=f"edge {dt.__name__} n_t0={cs['n_t0']}")
+    assert saw_null, "the long gaps must produce null cells in at least one case"
 
 
 # ---------------------------------------------------------------------------------------- periodic
@@ -261,10 +263,12 @@ def test_whole_path_against_oracle(cfg, n_random, torch_cuda, cetra, oracle_mod)
         phase_err = (t0_rec - i0["t0"] + 0.5 * i0["period"]) % i0["period"] - 0.5 * i0["period"]
         assert abs(phase_err) <= 0.1 * i0["duration"]
     else:
-        # cfg 1: a single transit; every period sees it once, at the injected epoch
+        # cfg 1: a single transit; the recovered first-epoch cell is the injected epoch modulo the best period
         i0 = p.injections[0]
         t0_rec = p.t0_start + pk["i_t0"][kb_g] * p.t0_stride
-        assert abs(t0_rec - i0["t0"]) <= 0.1 * i0["duration"]
+        pb = periods[kb_g]
+        phase_err = (t0_rec - i0["t0"] + 0.5 * pb) % pb - 0.5 * pb
+        assert abs(phase_err) <= 0.1 * i0["duration"]
 
 
 def test_config4_whole_path_sampled(torch_cuda, cetra, oracle_mod):
