@@ -71,6 +71,37 @@ __global__ void build_taps_kernel(const __grid_constant__ LinearParams P, const 
 }
 
 // ------------------------------------------------------------------------------------------- L2 + L3
+// Packed FP32 (FFMA2 / FADD2 on sm_100a): both sufficient statistics of a cell in one issue slot.  The two
+// halves are independent IEEE fp32 operations with round-to-nearest, exactly fmaf / + on each component.
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) {
+    float2 r;
+    asm("{\n\t"
+        ".reg .b64 ra, rb, rc, rd;\n\t"
+        "mov.b64 ra, {%2, %3};\n\t"
+        "mov.b64 rb, {%4, %5};\n\t"
+        "mov.b64 rc, {%6, %7};\n\t"
+        "fma.rn.f32x2 rd, ra, rb, rc;\n\t"
+        "mov.b64 {%0, %1}, rd;\n\t"
+        "}"
+        : "=f"(r.x), "=f"(r.y)
+        : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y), "f"(c.x), "f"(c.y));
+    return r;
+}
+
+__device__ __forceinline__ float2 add2f(float2 a, float2 b) {
+    float2 r;
+    asm("{\n\t"
+        ".reg .b64 ra, rb, rc;\n\t"
+        "mov.b64 ra, {%2, %3};\n\t"
+        "mov.b64 rb, {%4, %5};\n\t"
+        "add.rn.f32x2 rc, ra, rb;\n\t"
+        "mov.b64 {%0, %1}, rc;\n\t"
+        "}"
+        : "=f"(r.x), "=f"(r.y)
+        : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return r;
+}
+
 template <int R, int WARPS, bool Q1>
 __global__ void __launch_bounds__(WARPS * 32)
 linear_search_kernel(const __grid_constant__ LinearParams P) {
@@ -116,9 +147,9 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
     // kFlush*R terms before it is added to terms of its own size (cfg 3 has
     // windows of 2 701 points).
     constexpr int kFlush = 4;
-    float accA[R], accB[R], totA[R], totB[R];
+    float2 acc[R], tot[R];                                     // (S_wmf, S_wmm) of R consecutive t0 cells
 #pragma unroll
-    for (int r = 0; r < R; ++r) { accA[r] = 0.f; accB[r] = 0.f; totA[r] = 0.f; totB[r] = 0.f; }
+    for (int r = 0; r < R; ++r) { acc[r] = make_float2(0.f, 0.f); tot[r] = make_float2(0.f, 0.f); }
 
     const float2 *xs = data + d0 + q * (tid * R);
     for (int b = 0; b < q; ++b) {
@@ -141,9 +172,8 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
                 tap = tb[a0 + u + 1];
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
-                    const float2 x = win[(u + r) % R];
-                    accB[r] = fmaf(t.x, x.x, accB[r]);           // S_wmf += m   * (w f)
-                    accA[r] = fmaf(t.y, x.y, accA[r]);           // S_wmm += m^2 * w
+                    // S_wmf += m * (w f),  S_wmm += m^2 * w
+                    acc[r] = fma2(t, win[(u + r) % R], acc[r]);
                 }
             }
             if (Q1) xp += R;
@@ -151,8 +181,8 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
                 since_flush = 0;
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
-                    totA[r] += accA[r]; totB[r] += accB[r];
-                    accA[r] = 0.f; accB[r] = 0.f;
+                    tot[r] = add2f(tot[r], acc[r]);
+                    acc[r] = make_float2(0.f, 0.f);
                 }
             }
         }
@@ -161,7 +191,7 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
     // transpose through shared memory so that the global stores are coalesced
     float2 *st = stage + warp * (32 * R);
 #pragma unroll
-    for (int r = 0; r < R; ++r) st[lane * R + r] = make_float2(totA[r], totB[r]);
+    for (int r = 0; r < R; ++r) st[lane * R + r] = make_float2(tot[r].y, tot[r].x);   // stored as (S_wmm, S_wmf)
     __syncwarp();
     const long long row = lc * P.n_dur + j;
     const long long i_warp = i_blk + static_cast<long long>(warp) * (32 * R);
