@@ -66,6 +66,22 @@ def work_counts(p):
     return dict(template_evals=evals, pairs=pairs, gathers=pairs * p.n_t0, cells=p.n_t0 * len(p.durations))
 
 
+def rank_slice(rank: int, world: int, per_rank: int):
+    """Light curves [lo, hi) of the world*per_rank-curve batch that `rank` searches (weak scaling: curves are
+    independent, so the partition is the whole multi-GPU design; no data-path collective)."""
+    return rank * per_rank, (rank + 1) * per_rank
+
+
+def max_over_ranks(ms: float, device, world: int) -> float:
+    """Device-timed milliseconds -> the slowest rank's (the job finishes when the last rank does)."""
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons while the timed region runs (B200_PROFILING.md clocks line)."""
     FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -201,7 +217,7 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
         dist.init_process_group("nccl", device_id=dev)
 
     B = args.n_lc
-    p = make_survey_batch(n_lc=B * world, lc_range=(rank * B, (rank + 1) * B))   # each rank owns its curves
+    p = make_survey_batch(n_lc=B * world, lc_range=rank_slice(rank, world, B))   # each rank owns its curves
     wc = work_counts(p)
     K = p.periods.shape[0]
     flux_h = torch.from_numpy(p.flux).pin_memory()
@@ -248,11 +264,8 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
         prof = cetra.cetra_profile_read(reset=True) if profile else None
         if profile:
             cetra.cetra_profile_enable(False)
-        ms = sum(a.elapsed_time(b) for a, b in evs)
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item()), launches, prof, wall
+        ms = max_over_ranks(sum(a.elapsed_time(b) for a, b in evs), dev, world)
+        return ms, launches, prof, wall
 
     for _ in range(args.warmup):
         step_device()
