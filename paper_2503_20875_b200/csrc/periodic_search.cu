@@ -45,38 +45,78 @@ __device__ __forceinline__ float2 load_cell(const float2 *p) {
     return __ldg(p);
 }
 
+// Epoch offsets of one block of 32 epochs, as a warp holds them: lane l owns epoch eb + l.
+//   oa     off_e = llrint(e * r) of the lane's epoch (FP64, R11)
+//   dmask  bit l = off_{e+1} - off_e - floor(r)  (0 or 1 when `plain`)
+//   plain  every in-range step is floor(r) or floor(r)+1, so the warp can walk the offsets with
+//          off += floor(r) + bit: the inner loop then needs no shuffle (a SHFL costs a shared-memory
+//          wavefront, the resource this kernel is bound by).  Otherwise the offsets are broadcast by SHFL.
+struct EpochBlock {
+    long long oa;
+    int off0;           // offset of epoch eb (the same in every lane)
+    unsigned dmask;
+    bool plain;
+};
+
+__device__ __forceinline__ EpochBlock epoch_block(int eb, double r, long long r_floor, int n_t0, int lane) {
+    EpochBlock b;
+    const double e = static_cast<double>(eb + lane);
+    b.oa = __double2ll_rn(__dmul_rn(e, r));
+    const long long o0 = __double2ll_rn(__dmul_rn(static_cast<double>(eb), r));
+    b.off0 = static_cast<int>(o0 < 0x7fffffffLL ? o0 : 0x7fffffffLL);
+    const long long ob = __double2ll_rn(__dmul_rn(e + 1.0, r));
+    const long long dl = ob - b.oa - r_floor;
+    b.dmask = __ballot_sync(0xffffffffu, dl != 0);
+    b.plain = __ballot_sync(0xffffffffu, b.oa <= n_t0 - 1 && (dl < 0 || dl > 1)) == 0u;
+    return b;
+}
+
 // One pass of a warp over G*32 consecutive phases starting at p0: lane handles phases p0 + lane + 32 g.
 // Cells beyond n_t0-1 are zero (row padding), so epochs that run off the end for the later phases of the
 // pass add nothing; the epoch loop itself stops at the last epoch valid for p0.
 template <int G, bool kSmemRow>
 __device__ __forceinline__ void fold_pass(const float2 *__restrict__ row, int p0, int n_t0, int n_phase, double r,
-                                          int lane, float &best_lr, int &best_p) {
+                                          long long r_floor, const EpochBlock &b0, int lane, float &best_lr,
+                                          int &best_p) {
     float2 acc[G];
 #pragma unroll
     for (int g = 0; g < G; ++g) acc[g] = make_float2(0.f, 0.f);
     const long long limit = static_cast<long long>(n_t0) - 1 - p0;     // off_e <= limit  <=>  p0 + off_e <= I-1
     const float2 *base = row + p0 + lane;
+    const int step = static_cast<int>(r_floor < 0x3fffffffLL ? r_floor : 0x3fffffffLL);
+    EpochBlock b = b0;
     for (int eb = 0;; eb += 32) {
-        const long long off_ll = __double2ll_rn(__dmul_rn(static_cast<double>(eb + lane), r));   // R11
-        const bool ok = off_ll <= limit;
-        const int my_off = ok ? static_cast<int>(off_ll) : 0;
+        if (eb > 0) b = epoch_block(eb, r, r_floor, n_t0, lane);
+        const bool ok = b.oa <= limit;
         const int cnt = __popc(__ballot_sync(0xffffffffu, ok));      // offsets are monotone in e: valid ones are a prefix
+        if (b.plain) {
+            int off = b.off0;
+            unsigned m = b.dmask;
 #pragma unroll 4
-        for (int t = 0; t < cnt; ++t) {
-            const int off = __shfl_sync(0xffffffffu, my_off, t);
-            const float2 *ptr = base + off;
+            for (int t = 0; t < cnt; ++t) {
+                const float2 *ptr = base + off;
 #pragma unroll
-            for (int g = 0; g < G; ++g) acc[g] = add2(acc[g], load_cell<kSmemRow>(ptr + 32 * g));
+                for (int g = 0; g < G; ++g) acc[g] = add2(acc[g], load_cell<kSmemRow>(ptr + 32 * g));
+                off += step + static_cast<int>(m & 1u);
+                m >>= 1;
+            }
+        } else {
+            const int my_off = ok ? static_cast<int>(b.oa) : 0;
+            for (int t = 0; t < cnt; ++t) {
+                const float2 *ptr = base + __shfl_sync(0xffffffffu, my_off, t);
+#pragma unroll
+                for (int g = 0; g < G; ++g) acc[g] = add2(acc[g], load_cell<kSmemRow>(ptr + 32 * g));
+            }
         }
         if (cnt < 32) break;
     }
 #pragma unroll
     for (int g = 0; g < G; ++g) {
         const int p = p0 + lane + 32 * g;
-        const float a = acc[g].x, b = acc[g].y;
+        const float a = acc[g].x, bsum = acc[g].y;
         // candidate iff some epoch contributed (S_wmm > 0); selection uses an approximate reciprocal,
         // the reported values are recomputed with IEEE division by finalize_peaks_kernel
-        const float lr = 0.5f * b * b * rcp_approx(a);
+        const float lr = 0.5f * bsum * bsum * rcp_approx(a);
         if (p < n_phase && a > 0.f && lr > best_lr) { best_lr = lr; best_p = p; }
     }
 }
@@ -86,16 +126,18 @@ __device__ __forceinline__ void fold_period(const float2 *__restrict__ row, int 
                                             float &best_lr, int &best_p) {
     best_lr = -1.f;
     best_p = 0x7fffffff;
+    const long long r_floor = __double2ll_rd(r);
+    const EpochBlock b0 = epoch_block(0, r, r_floor, n_t0, lane);   // the first 32 epochs serve every pass
     int p0 = 0;
     for (; p0 + 32 * kFoldR <= n_phase; p0 += 32 * kFoldR)
-        fold_pass<kFoldR, kSmemRow>(row, p0, n_t0, n_phase, r, lane, best_lr, best_p);
+        fold_pass<kFoldR, kSmemRow>(row, p0, n_t0, n_phase, r, r_floor, b0, lane, best_lr, best_p);
     static_assert(kFoldR == 4, "the remainder switch below covers 1..kFoldR groups");
     const int groups = (n_phase - p0 + 31) >> 5;
     switch (groups) {
-        case 1: fold_pass<1, kSmemRow>(row, p0, n_t0, n_phase, r, lane, best_lr, best_p); break;
-        case 2: fold_pass<2, kSmemRow>(row, p0, n_t0, n_phase, r, lane, best_lr, best_p); break;
-        case 3: fold_pass<3, kSmemRow>(row, p0, n_t0, n_phase, r, lane, best_lr, best_p); break;
-        case 4: fold_pass<4, kSmemRow>(row, p0, n_t0, n_phase, r, lane, best_lr, best_p); break;   // 97..127 phases left
+        case 1: fold_pass<1, kSmemRow>(row, p0, n_t0, n_phase, r, r_floor, b0, lane, best_lr, best_p); break;
+        case 2: fold_pass<2, kSmemRow>(row, p0, n_t0, n_phase, r, r_floor, b0, lane, best_lr, best_p); break;
+        case 3: fold_pass<3, kSmemRow>(row, p0, n_t0, n_phase, r, r_floor, b0, lane, best_lr, best_p); break;
+        case 4: fold_pass<4, kSmemRow>(row, p0, n_t0, n_phase, r, r_floor, b0, lane, best_lr, best_p); break;   // 97..127 phases left
         default: break;
     }
     // warp argmax: larger lr wins, ties -> smaller phase
@@ -107,11 +149,14 @@ __device__ __forceinline__ void fold_period(const float2 *__restrict__ row, int 
     }
 }
 
+// Persistent CTAs claim contiguous ranges of work units (unit = kWarps consecutive periods of one row, one
+// period per warp) from a global counter, guided self-scheduling: a claim is 1/(2 x CTAs) of what is left,
+// so a CTA loads a row a handful of times per launch and the tail still balances.
 template <bool kSmemRow>
 __global__ void __launch_bounds__(kFoldThreads, 1) fold_argmax_kernel(const __grid_constant__ PeriodicParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
-    unsigned int *s_seg = reinterpret_cast<unsigned int *>(smem_raw + 8);
+    unsigned int *s_claim = reinterpret_cast<unsigned int *>(smem_raw + 8);
     float2 *srow = reinterpret_cast<float2 *>(smem_raw + 16);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int kWarps = kFoldThreads / 32;
@@ -124,46 +169,58 @@ __global__ void __launch_bounds__(kFoldThreads, 1) fold_argmax_kernel(const __gr
     long long cur_row = -1;
     uint32_t parity = 0;
     for (;;) {
-        if (tid == 0) *s_seg = atomicAdd(P.counter, 1u);
-        __syncthreads();
-        const long long seg = *s_seg;
-        __syncthreads();                       // everyone has read the slot and is done with the previous row
-        if (seg >= P.n_segs) break;
-        const long long rowid = seg / P.segs_per_row;              // lc * n_dur + j
-        const int s = static_cast<int>(seg - rowid * P.segs_per_row);
-        const int j = static_cast<int>(rowid % P.n_dur);
-        const long long lc = rowid / P.n_dur;
-        const float2 *grow = P.stats + rowid * P.stats_pitch;
-        if (kSmemRow && rowid != cur_row) {
-            if (tid == 0) {
-                const uint32_t bytes = static_cast<uint32_t>(P.stats_pitch) * 8u;
-                mbar_arrive_expect_tx(bar, bytes);
-                bulk_copy_g2s_chunked(srow, grow, bytes, bar);
-            }
-            mbar_wait(bar, parity);
-            parity ^= 1u;
-            cur_row = rowid;
+        if (tid == 0) {
+            const long long seen = *reinterpret_cast<volatile unsigned int *>(P.counter);   // may be stale: only sizes the claim
+            long long want = (P.n_units - seen) / (2LL * gridDim.x);
+            want = want < 1 ? 1 : (want > P.max_claim ? P.max_claim : want);
+            s_claim[0] = atomicAdd(P.counter, static_cast<unsigned int>(want));
+            s_claim[1] = static_cast<unsigned int>(want);
         }
-        const float2 *row = kSmemRow ? srow : grow;
-        const double D = P.durations[j];
-        const int k_end = min(P.n_per, (s + 1) * P.seg_len);
-        for (int k = s * P.seg_len + warp; k < k_end; k += kWarps) {
-            const double period = P.periods[k];
-            if (!(D < period)) continue;                            // overlapping windows are invalid
-            if (P.dur_lo && (j < P.dur_lo[k] || j >= P.dur_hi[k])) continue;
-            const double r = __ddiv_rn(period, P.t0_stride);        // period in t0 cells, FP64 (R11)
-            const double rc = ceil(r);
-            const int n_phase = rc < static_cast<double>(P.n_t0) ? static_cast<int>(rc) : P.n_t0;   // R10
-            float best_lr;
-            int best_p;
-            fold_period<kSmemRow>(row, P.n_t0, r, n_phase, lane, best_lr, best_p);
-            if (lane == 0 && best_lr >= 0.f) {
-                const unsigned int id = static_cast<unsigned int>(j) * static_cast<unsigned int>(P.n_t0) +
-                                        static_cast<unsigned int>(best_p);
-                const unsigned long long key =
-                    (static_cast<unsigned long long>(__float_as_uint(best_lr)) << 32) | (0xffffffffu - id);
-                atomicMax(P.keys + lc * P.n_per + k, key);
+        __syncthreads();
+        long long u = s_claim[0];
+        const long long u_end = min(u + static_cast<long long>(s_claim[1]), P.n_units);
+        __syncthreads();                       // everyone has read the slot and is done with the previous claim
+        if (u >= P.n_units) break;
+        while (u < u_end) {
+            const long long rowid = u / P.units_per_row;               // lc * n_dur + j
+            const long long u_row0 = rowid * P.units_per_row;
+            const long long u_stop = min(u_end, u_row0 + P.units_per_row);
+            const int j = static_cast<int>(rowid % P.n_dur);
+            const long long lc = rowid / P.n_dur;
+            const float2 *grow = P.stats + rowid * P.stats_pitch;
+            if (kSmemRow && rowid != cur_row) {
+                __syncthreads();               // every warp is done with the row about to be overwritten
+                if (tid == 0) {
+                    const uint32_t bytes = static_cast<uint32_t>(P.stats_pitch) * 8u;
+                    mbar_arrive_expect_tx(bar, bytes);
+                    bulk_copy_g2s_chunked(srow, grow, bytes, bar);
+                }
+                mbar_wait(bar, parity);
+                parity ^= 1u;
+                cur_row = rowid;
             }
+            const float2 *row = kSmemRow ? srow : grow;
+            const double D = P.durations[j];
+            const int k_end = static_cast<int>(min(static_cast<long long>(P.n_per), (u_stop - u_row0) * kWarps));
+            for (int k = static_cast<int>(u - u_row0) * kWarps + warp; k < k_end; k += kWarps) {
+                const double period = P.periods[k];
+                if (!(D < period)) continue;                            // overlapping windows are invalid
+                if (P.dur_lo && (j < P.dur_lo[k] || j >= P.dur_hi[k])) continue;
+                const double r = __ddiv_rn(period, P.t0_stride);        // period in t0 cells, FP64 (R11)
+                const double rc = ceil(r);
+                const int n_phase = rc < static_cast<double>(P.n_t0) ? static_cast<int>(rc) : P.n_t0;   // R10
+                float best_lr;
+                int best_p;
+                fold_period<kSmemRow>(row, P.n_t0, r, n_phase, lane, best_lr, best_p);
+                if (lane == 0 && best_lr >= 0.f) {
+                    const unsigned int id = static_cast<unsigned int>(j) * static_cast<unsigned int>(P.n_t0) +
+                                            static_cast<unsigned int>(best_p);
+                    const unsigned long long key =
+                        (static_cast<unsigned long long>(__float_as_uint(best_lr)) << 32) | (0xffffffffu - id);
+                    atomicMax(P.keys + lc * P.n_per + k, key);
+                }
+            }
+            u = u_stop;
         }
     }
 }
@@ -251,18 +308,15 @@ int build_periodic_plan(int32_t n_lc, int32_t n_dur, cetra_t0_grid grid, const d
     const size_t row_bytes = static_cast<size_t>(P.stats_pitch) * sizeof(float2);
     pl->row_in_smem = row_bytes + 16 <= static_cast<size_t>(smem_limit);
     pl->smem_bytes = pl->row_in_smem ? row_bytes + 16 : 16;
-    // period segments: a multiple of the warps per block so that every warp folds the same number of
-    // periods; shorter segments when the problem would otherwise not fill the chip
+    // work units: kWarps consecutive periods of one row (one period per warp); see fold_argmax_kernel
     const long long rows = static_cast<long long>(n_lc) * n_dur;
     constexpr int kWarps = kFoldThreads / 32;
-    int seg_len = 4 * kWarps;
-    while (seg_len > kWarps && rows * ((n_per + seg_len - 1) / seg_len) < 8LL * n_sm) seg_len /= 2;
-    P.seg_len = seg_len;
-    P.segs_per_row = (n_per + seg_len - 1) / seg_len;
-    P.n_segs = rows * P.segs_per_row;
-    if (P.n_segs > 0x7fffffffLL - 4096) return CETRA_ERR_UNSUPPORTED;
+    P.units_per_row = (n_per + kWarps - 1) / kWarps;
+    P.n_units = rows * P.units_per_row;
+    if (P.n_units > 0x7fffffffLL - (1LL << 24)) return CETRA_ERR_UNSUPPORTED;   // 32-bit queue head + overshoot
+    P.max_claim = std::max(1, 4 * P.units_per_row);
     const int per_sm = (pl->smem_bytes * 2 + 2048 <= static_cast<size_t>(smem_limit)) ? 2 : 1;
-    pl->grid = static_cast<int>(std::min<long long>(P.n_segs, static_cast<long long>(n_sm) * per_sm));
+    pl->grid = static_cast<int>(std::min<long long>(P.n_units, static_cast<long long>(n_sm) * per_sm));
     return CETRA_OK;
 }
 

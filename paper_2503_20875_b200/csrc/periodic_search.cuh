@@ -13,12 +13,12 @@ struct PeriodicParams {
     const double *periods;           // [n_per] device
     const int *dur_lo, *dur_hi;      // [n_per] device or null
     unsigned long long *keys;        // [n_lc][n_per] packed (lr bits << 32 | ~cell id), 0 = no candidate
-    unsigned int *counter;           // segment queue head
+    unsigned int *counter;           // work-unit queue head
     long long stats_pitch;
     double t0_start, t0_stride;
     int n_lc, n_dur, n_t0, n_per;
-    int segs_per_row, seg_len;
-    long long n_segs;
+    int units_per_row, max_claim;    // unit = kFoldThreads/32 consecutive periods of one row
+    long long n_units;
     double durations[CETRA_MAX_DURATIONS];
 };
 
