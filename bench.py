@@ -38,6 +38,9 @@ UNIT = "light curves/s"
 L2_FLUSH_BYTES = 512 << 20
 N_SM, FP32_LANES = 148, 128          # B200: SMs, FP32 FMA lanes per SM (B200_PROFILING.md unit counts)
 SMEM_BYTES_PER_CLK = 128             # shared-memory crossbar bytes/clk/SM (B300_MICROARCH.md, LDS/STS)
+# dram__bytes_read.sum + dram__bytes_write.sum of one fold_argmax_kernel launch over a 14-curve chunk of this
+# workload, from the `ncu --set full` capture summarised in profiles/r01c_fold_full.md (69.4 MB + 3.2 MB)
+NCU_FOLD_DRAM_BYTES_PER_LC = 72.6e6 / 14
 
 
 # ----------------------------------------------------------------------------------------------- helpers
@@ -305,7 +308,10 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
         gpu_launches=int(launches),
         clocks=clocks.summary(),
         roofline=dict(bound="hbm", kernel="fold_argmax_kernel", achieved=fold_gbs, peak=peaks["hbm_gbs"],
-                      unit="GB/s", frac=fold_gbs / peaks["hbm_gbs"], traffic=None, peak_source=peaks["source"],
+                      unit="GB/s", frac=fold_gbs / peaks["hbm_gbs"],
+                      traffic=NCU_FOLD_DRAM_BYTES_PER_LC * B * args.steps / fold_launches,
+                      traffic_source="ncu --set full, profiles/r01c_fold_full.md, scaled to the curves per launch",
+                      peak_source=peaks["source"],
                       ms_per_launch=prof["fold_ms"] / fold_launches, launches=int(prof["fold_launches"]),
                       share_of_step=prof["fold_ms"] / ms_dev,
                       algorithmic_bytes_per_launch=fold_bytes / fold_launches,
