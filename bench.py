@@ -227,7 +227,7 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
     err_h = torch.from_numpy(p.flux_err).pin_memory()
     flux_d, err_d = flux_h.to(dev), err_h.to(dev)
     gargs = (p.durations, p.t0_start, p.t0_stride, p.n_t0, p.template, p.periods)
-    ws_bytes = cetra.cetra_search_batched_host_workspace_bytes(p.times, B, 0, cetra.CETRA_F32, p.durations,
+    ws_bytes = cetra.cetra_search_batched_host_workspace_bytes(p.times, B, args.lc_chunk, cetra.CETRA_F32, p.durations,
                                                                p.t0_start, p.t0_stride, p.n_t0, len(p.template), K)
     ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
     peaks_d = torch.empty((B, K, 8), dtype=torch.int32, device=dev)
@@ -236,10 +236,11 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
     stream = torch.cuda.current_stream()
 
     def step_device():
-        cetra.cetra_search_batched(p.times, flux_d, err_d, *gargs, workspace=ws, peaks=peaks_d)
+        cetra.cetra_search_batched(p.times, flux_d, err_d, *gargs, lc_chunk=args.lc_chunk, workspace=ws, peaks=peaks_d)
 
     def step_host():
-        cetra.cetra_search_batched_host(p.times, flux_h, err_h, *gargs, workspace=ws, peaks_host=peaks_h, device=dev)
+        cetra.cetra_search_batched_host(p.times, flux_h, err_h, *gargs, lc_chunk=args.lc_chunk, workspace=ws,
+                                        peaks_host=peaks_h, device=dev)
 
     def barrier():
         if world > 1:
@@ -392,6 +393,7 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="sector", choices=["sector", "survey"])
     ap.add_argument("--n-lc", type=int, default=64, help="light curves per GPU per step (survey: per slice)")
+    ap.add_argument("--lc-chunk", type=int, default=0, help="light curves resident at a time (0 = library default)")
     ap.add_argument("--survey-lc", type=int, default=10000)
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU budget of the cpu_baseline sample")
     ap.add_argument("--ref-seconds", type=float, default=8.0, help="CPU budget of one --impl reference step")
