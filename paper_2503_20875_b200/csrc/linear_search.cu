@@ -152,8 +152,6 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
     for (int r = 0; r < R; ++r) { acc[r] = make_float2(0.f, 0.f); tot[r] = make_float2(0.f, 0.f); }
 
     const float2 *xs = data + d0 + q * (tid * R);
-    const int A_used = P.A_used[j];                             // taps per branch that can be non-zero (<= A)
-    const int A_full = A_used / R * R;
     for (int b = 0; b < q; ++b) {
         const float2 *xb = xs + b;
         const float2 *tb = taps + b * A;
@@ -164,7 +162,7 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
         float2 tap = tb[0];
         const float2 *xp = xb + q * R;
         int since_flush = 0;
-        for (int a0 = 0; a0 < A_full; a0 += R) {
+        for (int a0 = 0; a0 < A; a0 += R) {
 #pragma unroll
             for (int u = 0; u < R; ++u) {
                 win[(u + R - 1) % R] = nxt;
@@ -179,7 +177,7 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
                 }
             }
             if (Q1) xp += R;
-            if (++since_flush == kFlush) {
+            if (++since_flush == kFlush || a0 + R >= A) {
                 since_flush = 0;
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
@@ -187,24 +185,6 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
                     acc[r] = make_float2(0.f, 0.f);
                 }
             }
-        }
-        // the last, partial group of taps: the same rotation, left as soon as the taps run out (block-uniform)
-        const int rem = A_used - A_full;
-#pragma unroll
-        for (int u = 0; u < R; ++u) {
-            if (u >= rem) break;
-            win[(u + R - 1) % R] = nxt;
-            const float2 t = tap;
-            nxt = Q1 ? xp[u] : *xp;
-            if (!Q1) xp += q;
-            tap = tb[A_full + u + 1];
-#pragma unroll
-            for (int r = 0; r < R; ++r) acc[r] = fma2(t, win[(u + r) % R], acc[r]);
-        }
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            tot[r] = add2f(tot[r], acc[r]);
-            acc[r] = make_float2(0.f, 0.f);
         }
     }
 
@@ -274,7 +254,6 @@ int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const d
         const int ntap = 2 * P.H[j] + 1;
         const int per_phase = (ntap + P.q - 1) / P.q;
         P.A[j] = (per_phase + R - 1) / R * R;
-        P.A_used[j] = per_phase;
         P.durations[j] = D;
         const long long stored = (static_cast<long long>(P.q) * P.A[j] + 2 + 1) & ~1LL;   // +2: prefetch overrun
         if (P.tap_off[j] + stored > 0x7fffffffLL) return CETRA_ERR_UNSUPPORTED;
@@ -289,19 +268,19 @@ int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const d
     std::stable_sort(ord.begin(), ord.end(), [&](int a, int b) { return P.A[a] > P.A[b]; });
     for (int j = 0; j < n_dur; ++j) P.order[j] = static_cast<unsigned char>(ord[j]);
 
-    // tile shape: among 4, 3, 2, 1 warps per block (tile = warps*32*R cells) the one that wastes the fewest
-    // cells in the last tile of a row, provided it fits in shared memory and the grid fills the chip
-    int warps = 0;
-    long long best_padded = 0;
-    for (int w = 4; w >= 1; --w) {
-        const int tile = w * 32 * R;
+    // tile shape: as many warps per block as shared memory allows, fewer when the grid would not fill the chip
+    int warps = 4;
+    for (;;) {
+        const int tile = warps * 32 * R;
         const long long tiles = (grid.n_t0 + tile - 1) / tile;
         const long long blocks = tiles * n_dur * n_lc;
-        const bool fits = linear_smem_bytes(*pl, R, w) <= static_cast<size_t>(smem_limit);
-        if (!fits || (blocks < 2LL * n_sm && w > 1)) continue;
-        if (warps == 0 || tiles * tile < best_padded) { warps = w; best_padded = tiles * tile; }
+        const bool fits = linear_smem_bytes(*pl, R, warps) <= static_cast<size_t>(smem_limit);
+        if (warps == 1 || (fits && blocks >= 2LL * n_sm)) {
+            if (!fits) return CETRA_ERR_UNSUPPORTED;
+            break;
+        }
+        warps /= 2;
     }
-    if (warps == 0) return CETRA_ERR_UNSUPPORTED;
     pl->warps = warps;
     pl->tile = warps * 32 * R;
     P.tiles_per_row = static_cast<int>((grid.n_t0 + pl->tile - 1) / pl->tile);
@@ -387,7 +366,6 @@ int run_linear(LinearPlan &pl, const void *flux_dev, const void *flux_err_dev, c
     int rc;
     switch (pl.warps) {
         case 4: rc = launch_linear<R, 4>(pl, P, blocks, st); break;
-        case 3: rc = launch_linear<R, 3>(pl, P, blocks, st); break;
         case 2: rc = launch_linear<R, 2>(pl, P, blocks, st); break;
         default: rc = launch_linear<R, 1>(pl, P, blocks, st); break;
     }

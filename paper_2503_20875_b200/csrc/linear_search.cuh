@@ -16,8 +16,7 @@ struct LinearParams {
     long long lc_pitch, n_lo, n0, n_t0, stats_pitch;
     int q, n_dur, tiles_per_row;
     int H[CETRA_MAX_DURATIONS];         // window half-reach in samples (superset of the window)
-    int A[CETRA_MAX_DURATIONS];         // taps per polyphase branch, padded to a multiple of kLinearR (table stride)
-    int A_used[CETRA_MAX_DURATIONS];    // taps per polyphase branch inside the window superset (<= A)
+    int A[CETRA_MAX_DURATIONS];         // taps per polyphase branch, padded to a multiple of kLinearR
     int tap_off[CETRA_MAX_DURATIONS + 1];
     unsigned char order[CETRA_MAX_DURATIONS];
     double durations[CETRA_MAX_DURATIONS];
