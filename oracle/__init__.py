@@ -16,15 +16,17 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "cetra_oracle.c")
+_SRC_SETUP = os.path.join(_HERE, "cetra_oracle_setup.c")
 _LIB = os.path.join(_HERE, "libcetra_oracle.so")
 _lib: Optional[ctypes.CDLL] = None
 
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc.  -ffp-contract=off keeps every FP64 operation a plain IEEE one."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    newest = max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_SETUP))
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < newest:
         cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC",
-               _SRC, "-o", _LIB, "-lm"]
+               _SRC, _SRC_SETUP, "-o", _LIB, "-lm"]
         subprocess.run(cmd, check=True)
     return _LIB
 
@@ -49,6 +51,17 @@ def _load() -> ctypes.CDLL:
         lib.oracle_periodic_cell.argtypes = [dp, dp, dp, ctypes.c_int32, ctypes.c_int64, ctypes.c_double,
                                              ctypes.c_double, ctypes.c_int32, ctypes.c_int64,
                                              dp, dp, dp, ip]
+        lib.oracle_median_cadence.restype = ctypes.c_int
+        lib.oracle_median_cadence.argtypes = [dp, ctypes.c_int64, dp]
+        lib.oracle_resample.restype = ctypes.c_int
+        lib.oracle_resample.argtypes = [dp, dp, dp, ctypes.c_int64, ctypes.c_double, ctypes.c_double,
+                                        ctypes.c_int64, dp, dp]
+        lib.oracle_monotransit.restype = ctypes.c_int
+        lib.oracle_monotransit.argtypes = [dp, dp, dp, ctypes.c_int32, ctypes.c_int64, ctypes.c_double, dp,
+                                           ctypes.c_int32, ctypes.c_double, dp, ip, lp, ip, dp, dp, dp, ip]
+        lib.oracle_mask_transits.restype = ctypes.c_int
+        lib.oracle_mask_transits.argtypes = [dp, dp, ctypes.c_int64, ctypes.c_double, ctypes.c_double,
+                                             ctypes.c_double, ctypes.c_double, lp]
         lib.oracle_set_threads.argtypes = [ctypes.c_int]
         lib.oracle_get_threads.restype = ctypes.c_int
         _lib = lib
@@ -142,3 +155,72 @@ def periodic_cell(grids: LinearGrids, t0_stride: float, period: float, j: int, p
     if rc != 0:
         raise ValueError(f"oracle_periodic_cell failed with status {rc}")
     return lr.value, z.value, zv.value, ntr.value
+
+
+# ------------------------------------------------------------------------- setup and follow-up steps
+def median_cadence(times) -> float:
+    """Default resample cadence: the median cadence of the input (R22)."""
+    lib = _load()
+    times = _d(times)
+    out = ctypes.c_double()
+    rc = lib.oracle_median_cadence(_p(times, ctypes.c_double), times.shape[0], ctypes.byref(out))
+    if rc != 0:
+        raise ValueError(f"oracle_median_cadence failed with status {rc}")
+    return out.value
+
+
+def resample(times, flux, flux_err, t_start: float, cadence: float, n_out: int):
+    """Irregular light curve -> regular grid (R21): (flux[n_out], flux_err[n_out])."""
+    lib = _load()
+    times, flux, flux_err = map(_d, (times, flux, flux_err))
+    of, oe = np.empty(n_out), np.empty(n_out)
+    c = ctypes.c_double
+    rc = lib.oracle_resample(_p(times, c), _p(flux, c), _p(flux_err, c), times.shape[0], float(t_start),
+                             float(cadence), int(n_out), _p(of, c), _p(oe, c))
+    if rc != 0:
+        raise ValueError(f"oracle_resample failed with status {rc}")
+    return of, oe
+
+
+@dataclass
+class Monotransits:
+    """Single-transit events of the linear-search output (R23)."""
+    profile_lr: np.ndarray      # [I] max over durations of dlogL
+    profile_j: np.ndarray       # [I] its duration index (-1: every duration null)
+    i_t0: np.ndarray            # [n_found]
+    j_dur: np.ndarray
+    lr: np.ndarray
+    depth: np.ndarray
+    depth_var: np.ndarray
+
+
+def monotransit(grids: LinearGrids, t0_stride: float, durations, n_peaks: int, excl: float = 1.0) -> Monotransits:
+    lib = _load()
+    depth, var, dl = _d(grids.depth), _d(grids.depth_var), _d(grids.dlogL)
+    durations = _d(durations)
+    nj, ni = depth.shape
+    c, i32, i64 = ctypes.c_double, ctypes.c_int32, ctypes.c_int64
+    pl, pj = np.empty(ni), np.empty(ni, np.int32)
+    ei, ej = np.empty(n_peaks, np.int64), np.empty(n_peaks, np.int32)
+    el, ed, ev = np.empty(n_peaks), np.empty(n_peaks), np.empty(n_peaks)
+    nf = ctypes.c_int32()
+    rc = lib.oracle_monotransit(_p(depth, c), _p(var, c), _p(dl, c), nj, ni, float(t0_stride), _p(durations, c),
+                                int(n_peaks), float(excl), _p(pl, c), _p(pj, i32), _p(ei, i64), _p(ej, i32),
+                                _p(el, c), _p(ed, c), _p(ev, c), ctypes.byref(nf))
+    if rc != 0:
+        raise ValueError(f"oracle_monotransit failed with status {rc}")
+    n = nf.value
+    return Monotransits(pl, pj, ei[:n], ej[:n], el[:n], ed[:n], ev[:n])
+
+
+def mask_transits(times, flux, period: float, t0: float, duration: float, width: float = 1.0):
+    """Copy of `flux` with the samples within width*D/2 of a transit mid-time set to NaN (R24)."""
+    lib = _load()
+    times = _d(times)
+    out = _d(flux).copy()
+    cnt = ctypes.c_int64()
+    rc = lib.oracle_mask_transits(_p(times, ctypes.c_double), _p(out, ctypes.c_double), times.shape[0],
+                                  float(period), float(t0), float(duration), float(width), ctypes.byref(cnt))
+    if rc != 0:
+        raise ValueError(f"oracle_mask_transits failed with status {rc}")
+    return out, cnt.value
