@@ -16,6 +16,7 @@ from .lightcurves import (  # noqa: F401
     tabulate_template,
     make_config,
     make_survey_batch,
+    make_irregular_batch,
     duration_grid,
     period_grid_uniform_frequency,
     CONFIG_NAMES,

@@ -278,3 +278,43 @@ def make_survey_batch(n_lc: int = 10000, n_periods: Optional[int] = None,
         durations=durations, t0_start=t0_start, t0_stride=stride, n_t0=n_t0, periods=periods,
         injections=injections, meta=dict(seed=BASE_SEED + 5 + seed_offset, n_lc=n_lc, lc_range=lc_range),
     )
+
+
+# --------------------------------------------------------------------------
+# Irregularly sampled input for the resampler (PLATO camera-group averages, barycentric times)
+# --------------------------------------------------------------------------
+def make_irregular_batch(seed: int = 250320881, n_lc: int = 3, n: int = 6000, cadence_s: float = 120.0,
+                         dtype=np.float32, shuffle: bool = True):
+    """`n_lc` light curves sharing one irregular timestamp array: a 2-min clock with a slow barycentric drift
+    and per-point jitter, 3 % of the points dropped, a 0.4 d gap, 10 % extra "second camera group" points
+    half a minute after their partner, a few null observations; optionally in shuffled order.
+    Returns (times [n_obs] float64, flux [n_lc][n_obs], flux_err [n_lc][n_obs])."""
+    rng = np.random.default_rng(seed)
+    c = cadence_s / 86400.0
+    t = 1325.0 + c * np.arange(n) + 2.0e-4 * np.sin(np.arange(n) * c * 2 * np.pi / 27.0) \
+        + rng.uniform(-0.2, 0.2, n) * c
+    keep = rng.random(n) > 0.03
+    keep &= ~((t > t[0] + 3.1) & (t < t[0] + 3.5))
+    t = t[keep]
+    extra = t[rng.random(t.shape[0]) < 0.10] + 0.25 * c
+    t = np.concatenate([t, extra])
+    if shuffle:
+        t = t[rng.permutation(t.shape[0])]
+    n_obs = t.shape[0]
+    sig = rng.uniform(4e-4, 1.5e-3, (n_lc, n_obs))
+    flux = 1.0 + sig * rng.standard_normal((n_lc, n_obs))
+    for b in range(n_lc):
+        flux[b] -= _inject_profile(t, period=1.3 + 0.4 * b, t0=t.min() + 0.5, depth=2e-3, duration=0.1)
+    bad = rng.random((n_lc, n_obs)) < 0.01
+    flux[bad] = np.nan
+    sig[rng.random((n_lc, n_obs)) < 0.005] = np.inf
+    return t.astype(np.float64), flux.astype(dtype), sig.astype(dtype)
+
+
+def _inject_profile(t: np.ndarray, period: float, t0: float, depth: float, duration: float) -> np.ndarray:
+    ph = np.mod(t - t0 + 0.5 * period, period) - 0.5 * period
+    x = ph / duration + 0.5
+    out = np.zeros_like(t)
+    ins = (x >= 0.0) & (x <= 1.0)
+    out[ins] = depth * transit_profile(x[ins])
+    return out

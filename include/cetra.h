@@ -177,6 +177,91 @@ int cetra_search_batched_host(const double *times_host, const void *flux_host, c
                               cetra_peak *peaks_host,
                               void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
 
+/* ------------------------------------------------------------------------------------------
+ * Setup: light-curve resampling (§2.1.1, lines 53-61).
+ *
+ * cetra_median_cadence   host-only: the default resample cadence, the median of the differences of
+ *                        the time-sorted finite timestamps (R22).
+ * cetra_resample_grid    host-only: the regular output grid for `times_host`: cadence (<= 0: the median
+ *                        cadence), `pad_days` of null padding at both ends (half the maximum
+ *                        trial duration), rounded up to whole points.  Output point n is at
+ *                        t_start + n * cadence; the first observation falls on point ceil(pad/cadence).
+ * cetra_resample         every observation goes to the nearest output point,
+ *                        cell = floor((t - t_start)/cadence + 1/2) in FP64 (R21); observations sharing a
+ *                        point are combined with the inverse-variance weighted mean, error
+ *                        (sum 1/sigma^2)^-1/2; points without data get flux = NaN, flux_err = +inf
+ *                        (PAPER.md:55).  Null observations (non-finite time/flux/error, error <= 0) and
+ *                        observations off the grid are dropped.  The input needs no ordering.
+ *     times_dev              [n_in] float64 DEVICE (the irregular timestamps are a large array)
+ *     flux_dev, flux_err_dev [n_lc][n_in] dtype, sharing times_dev
+ *     flux_out_dev, flux_err_out_dev [n_lc][n_out] dtype (same dtype as the input); n_in = 0 gives an all-null grid
+ *     workspace              cetra_resample_workspace_bytes(n_lc, n_out): FP64 sums per output point
+ * The sums are FP64 atomics: the result does not depend on the order of the input beyond FP64 rounding.
+ * ------------------------------------------------------------------------------------------ */
+int cetra_median_cadence(const double *times_host, int64_t n, double *cadence);
+
+int cetra_resample_grid(const double *times_host, int64_t n, double cadence, double pad_days,
+                        double *t_start, double *cadence_out, int64_t *n_out);
+
+size_t cetra_resample_workspace_bytes(int32_t n_lc, int64_t n_out);
+
+int cetra_resample(const double *times_dev, const void *flux_dev, const void *flux_err_dev, cetra_dtype dtype,
+                   int64_t n_in, int32_t n_lc, double t_start, double cadence, int64_t n_out,
+                   void *flux_out_dev, void *flux_err_out_dev,
+                   void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* ------------------------------------------------------------------------------------------
+ * Monotransit search: single-transit events in the linear-search output alone.
+ *
+ *  profile(i) = max_j dlogL[j][i] (null cells skipped; ties: smallest j).  Events are taken greedily by
+ *  decreasing profile (ties: smallest i); an event at (i, j) removes every reference time with
+ *  |t - t_i| <= excl * D_j from further consideration (R23).
+ *
+ *  depth_dev, var_dev, dlogL_dev  [n_lc][n_dur][n_t0] float32, the linear-search grids
+ *  profile_lr_dev  optional [n_lc][n_t0] float32 (NaN where every duration is null)
+ *  profile_j_dev   optional [n_lc][n_t0] int32   (-1 there)
+ *  events_dev      [n_lc][n_peaks] records; entries beyond n_found are NaN / -1
+ *  n_found_dev     [n_lc] int32
+ * ------------------------------------------------------------------------------------------ */
+typedef struct {
+    float lr;           /* dlogL of the event (Eq. 2) */
+    float depth;
+    float depth_var;
+    float t0;           /* t0_start + i_t0 * t0_stride */
+    int32_t i_t0;
+    int32_t j_dur;
+    int32_t reserved[2];
+} cetra_event;
+
+size_t cetra_monotransit_workspace_bytes(int32_t n_lc, int64_t n_t0);
+
+int cetra_monotransit_search(const float *depth_dev, const float *var_dev, const float *dlogL_dev,
+                             int32_t n_lc, int32_t n_dur, cetra_t0_grid grid, const double *durations_host,
+                             int32_t n_peaks, double excl,
+                             float *profile_lr_dev, int32_t *profile_j_dev,
+                             cetra_event *events_dev, int32_t *n_found_dev,
+                             void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* ------------------------------------------------------------------------------------------
+ * Iterative masking: nullify the flux within and around a detected signal before the
+ * search is repeated.  Sample n of light curve b is set to NaN when its distance to the nearest transit
+ * mid-time t0[b] + e * period[b] (e any integer; period[b] <= 0: the single event at t0[b]) is
+ * <= width * duration[b] / 2 (R24), all in FP64.
+ *
+ *  times_dev       [n] float64 DEVICE
+ *  flux_dev        [n_lc][n] dtype, modified in place
+ *  period_host, t0_host, duration_host  [n_lc] float64 (a light curve with a non-finite t0 or a
+ *                  non-positive duration is left untouched)
+ *  n_masked_dev    optional [n_lc] int32: samples nullified by this call
+ *  workspace       cetra_mask_workspace_bytes(n_lc)
+ * ------------------------------------------------------------------------------------------ */
+size_t cetra_mask_workspace_bytes(int32_t n_lc);
+
+int cetra_mask_transits(const double *times_dev, void *flux_dev, cetra_dtype dtype, int64_t n, int32_t n_lc,
+                        const double *period_host, const double *t0_host, const double *duration_host,
+                        double width, int32_t *n_masked_dev,
+                        void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
 /* Number of kernel launches the library has enqueued since the process started (diagnostic). */
 int64_t cetra_kernel_launch_count(void);
 

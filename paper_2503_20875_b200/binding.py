@@ -33,6 +33,9 @@ EXPORTED_SYMBOLS = (
     "cetra_search_batched_workspace_bytes", "cetra_search_batched",
     "cetra_search_batched_host_workspace_bytes", "cetra_search_batched_host",
     "cetra_profile_enable", "cetra_profile_read",
+    "cetra_median_cadence", "cetra_resample_grid", "cetra_resample_workspace_bytes", "cetra_resample",
+    "cetra_monotransit_workspace_bytes", "cetra_monotransit_search",
+    "cetra_mask_workspace_bytes", "cetra_mask_transits",
 )
 
 
@@ -55,6 +58,17 @@ class cetra_peak(ctypes.Structure):
 PEAK_DTYPE = np.dtype([("lr", "<f4"), ("depth", "<f4"), ("depth_var", "<f4"), ("t0", "<f4"),
                        ("i_t0", "<i4"), ("j_dur", "<i4"), ("n_transits", "<i4"), ("reserved", "<i4")])
 assert PEAK_DTYPE.itemsize == ctypes.sizeof(cetra_peak) == 32
+
+
+class cetra_event(ctypes.Structure):
+    _fields_ = [("lr", ctypes.c_float), ("depth", ctypes.c_float), ("depth_var", ctypes.c_float),
+                ("t0", ctypes.c_float), ("i_t0", ctypes.c_int32), ("j_dur", ctypes.c_int32),
+                ("reserved", ctypes.c_int32 * 2)]
+
+
+EVENT_DTYPE = np.dtype([("lr", "<f4"), ("depth", "<f4"), ("depth_var", "<f4"), ("t0", "<f4"),
+                        ("i_t0", "<i4"), ("j_dur", "<i4"), ("reserved", "<i4", (2,))])
+assert EVENT_DTYPE.itemsize == ctypes.sizeof(cetra_event) == 32
 
 _lib: Optional[ctypes.CDLL] = None
 
@@ -100,6 +114,24 @@ def load_library() -> ctypes.CDLL:
     lib.cetra_search_batched_host.restype = ctypes.c_int
     lib.cetra_search_batched_host.argtypes = [dp, vp, vp, ctypes.c_int, i64, i32, i32, dp, i32, cetra_t0_grid, fp,
                                               i32, dp, i32, ip, ip, vp, vp, sz, vp]
+    lib.cetra_median_cadence.restype = ctypes.c_int
+    lib.cetra_median_cadence.argtypes = [dp, i64, dp]
+    lib.cetra_resample_grid.restype = ctypes.c_int
+    lib.cetra_resample_grid.argtypes = [dp, i64, ctypes.c_double, ctypes.c_double, dp, dp, ctypes.POINTER(i64)]
+    lib.cetra_resample_workspace_bytes.restype = sz
+    lib.cetra_resample_workspace_bytes.argtypes = [i32, i64]
+    lib.cetra_resample.restype = ctypes.c_int
+    lib.cetra_resample.argtypes = [vp, vp, vp, ctypes.c_int, i64, i32, ctypes.c_double, ctypes.c_double, i64,
+                                   vp, vp, vp, sz, vp]
+    lib.cetra_monotransit_workspace_bytes.restype = sz
+    lib.cetra_monotransit_workspace_bytes.argtypes = [i32, i64]
+    lib.cetra_monotransit_search.restype = ctypes.c_int
+    lib.cetra_monotransit_search.argtypes = [vp, vp, vp, i32, i32, cetra_t0_grid, dp, i32, ctypes.c_double,
+                                             vp, vp, vp, vp, vp, sz, vp]
+    lib.cetra_mask_workspace_bytes.restype = sz
+    lib.cetra_mask_workspace_bytes.argtypes = [i32]
+    lib.cetra_mask_transits.restype = ctypes.c_int
+    lib.cetra_mask_transits.argtypes = [vp, vp, ctypes.c_int, i64, i32, dp, dp, dp, ctypes.c_double, vp, vp, sz, vp]
     lib.cetra_profile_enable.restype = ctypes.c_int
     lib.cetra_profile_enable.argtypes = [i32]
     lib.cetra_profile_read.restype = ctypes.c_int
@@ -418,3 +450,115 @@ def cetra_search_batched_host(times, flux_host, flux_err_host, durations, t0_sta
                                            ws.numel(), _stream_ptr(torch, stream))
     _check(rc, "cetra_search_batched_host")
     return peaks_host.numpy().view(PEAK_DTYPE).reshape(n_lc, n_per)
+
+
+# ----------------------------------------------------------------------- setup and follow-up steps
+def cetra_median_cadence(times) -> float:
+    """Default resample cadence: host-only helper of the library."""
+    times = _f64(times)
+    out = ctypes.c_double()
+    _check(load_library().cetra_median_cadence(_dp(times), times.shape[0], ctypes.byref(out)), "cetra_median_cadence")
+    return out.value
+
+
+def cetra_resample_grid(times, cadence: float = 0.0, pad_days: float = 0.0):
+    """(t_start, cadence, n_out) of the regular grid for `times`; cadence <= 0: the median."""
+    times = _f64(times)
+    t_start, c, n_out = ctypes.c_double(), ctypes.c_double(), ctypes.c_int64()
+    _check(load_library().cetra_resample_grid(_dp(times), times.shape[0], float(cadence), float(pad_days),
+                                              ctypes.byref(t_start), ctypes.byref(c), ctypes.byref(n_out)),
+           "cetra_resample_grid")
+    return t_start.value, c.value, int(n_out.value)
+
+
+def cetra_resample(times_dev, flux, flux_err, t_start: float, cadence: float, n_out: int, workspace=None,
+                   stream=None):
+    """Irregular light curves [B][N_in] (or [N_in]) sharing `times_dev` -> (flux, flux_err) on the regular grid."""
+    torch = _torch()
+    lib = load_library()
+    flux, flux_err, n_lc, n_in = _dev_input(torch, flux, flux_err)
+    squeeze = flux.dim() == 1
+    if not (times_dev.is_cuda and times_dev.dtype == torch.float64 and times_dev.numel() == n_in):
+        raise TypeError("times_dev must be a float64 CUDA tensor with one entry per observation")
+    times_dev = times_dev.contiguous()
+    nbytes = int(lib.cetra_resample_workspace_bytes(n_lc, int(n_out)))
+    ws = _workspace(torch, nbytes, flux.device, workspace)
+    out_f = torch.empty((n_lc, int(n_out)), dtype=flux.dtype, device=flux.device)
+    out_e = torch.empty_like(out_f)
+    with torch.cuda.device(flux.device):
+        rc = lib.cetra_resample(times_dev.data_ptr(), flux.data_ptr(), flux_err.data_ptr(), _dtype_code(torch, flux),
+                                n_in, n_lc, float(t_start), float(cadence), int(n_out), out_f.data_ptr(),
+                                out_e.data_ptr(), ws.data_ptr(), ws.numel(), _stream_ptr(torch, stream))
+    _check(rc, "cetra_resample")
+    return (out_f[0], out_e[0]) if squeeze else (out_f, out_e)
+
+
+@dataclass
+class MonotransitResult:
+    """Outputs of cetra_monotransit_search: events [B][n_peaks] records (int32 view, see events_to_numpy),
+    n_found [B] int32, optional profile tensors [B][I]."""
+    events: object
+    n_found: object
+    profile_lr: object
+    profile_j: object
+
+
+def cetra_monotransit_search(depth, depth_var, dlogL, t0_start: float, t0_stride: float, durations, n_peaks: int,
+                             excl: float = 1.0, want_profile: bool = False, workspace=None,
+                             stream=None) -> MonotransitResult:
+    torch = _torch()
+    lib = load_library()
+    grids = []
+    for g in (depth, depth_var, dlogL):
+        if not (g.is_cuda and g.dtype == torch.float32):
+            raise TypeError("the linear-search grids must be float32 CUDA tensors")
+        grids.append(g.contiguous() if g.dim() == 3 else g.contiguous()[None])
+    n_lc, n_dur, n_t0 = (int(x) for x in grids[0].shape)
+    durations = _f64(durations)
+    if durations.shape[0] != n_dur:
+        raise CetraError(CETRA_ERR_INVALID_ARG, "cetra_monotransit_search: len(durations) != grids.shape[-2]")
+    dev = grids[0].device
+    nbytes = int(lib.cetra_monotransit_workspace_bytes(n_lc, n_t0))
+    ws = _workspace(torch, nbytes, dev, workspace)
+    events = torch.empty((n_lc, int(n_peaks), 8), dtype=torch.int32, device=dev)
+    n_found = torch.empty((n_lc,), dtype=torch.int32, device=dev)
+    pl = torch.empty((n_lc, n_t0), dtype=torch.float32, device=dev) if want_profile else None
+    pj = torch.empty((n_lc, n_t0), dtype=torch.int32, device=dev) if want_profile else None
+    ptr = lambda t: t.data_ptr() if t is not None else None
+    with torch.cuda.device(dev):
+        rc = lib.cetra_monotransit_search(grids[0].data_ptr(), grids[1].data_ptr(), grids[2].data_ptr(), n_lc, n_dur,
+                                          _grid(t0_start, t0_stride, n_t0), _dp(durations), int(n_peaks), float(excl),
+                                          ptr(pl), ptr(pj), events.data_ptr(), n_found.data_ptr(), ws.data_ptr(),
+                                          ws.numel(), _stream_ptr(torch, stream))
+    _check(rc, "cetra_monotransit_search")
+    return MonotransitResult(events, n_found, pl, pj)
+
+
+def events_to_numpy(events) -> np.ndarray:
+    """[B][n_peaks][8] int32 tensor of cetra_event records -> numpy structured array [B][n_peaks]."""
+    a = events.detach().cpu().contiguous().numpy()
+    return a.view(EVENT_DTYPE).reshape(a.shape[:-1])
+
+
+def cetra_mask_transits(times_dev, flux, period, t0, duration, width: float = 1.0, workspace=None, stream=None):
+    """Set the samples within width*D/2 of a transit mid-time to NaN, in place; returns the
+    per-curve count of nullified samples as an int32 CUDA tensor."""
+    torch = _torch()
+    lib = load_library()
+    if not (flux.is_cuda and flux.is_contiguous()):
+        raise TypeError("flux must be a contiguous CUDA tensor (it is modified in place)")
+    n_lc, n = (1, flux.shape[0]) if flux.dim() == 1 else (int(flux.shape[0]), int(flux.shape[1]))
+    if not (times_dev.is_cuda and times_dev.dtype == torch.float64 and times_dev.numel() == n):
+        raise TypeError("times_dev must be a float64 CUDA tensor with one entry per sample")
+    per, tt, dur = (_f64(np.atleast_1d(x)) for x in (period, t0, duration))
+    if not (per.shape[0] == tt.shape[0] == dur.shape[0] == n_lc):
+        raise CetraError(CETRA_ERR_INVALID_ARG, "cetra_mask_transits: one (period, t0, duration) per light curve")
+    nbytes = int(lib.cetra_mask_workspace_bytes(n_lc))
+    ws = _workspace(torch, nbytes, flux.device, workspace)
+    n_masked = torch.empty((n_lc,), dtype=torch.int32, device=flux.device)
+    with torch.cuda.device(flux.device):
+        rc = lib.cetra_mask_transits(times_dev.contiguous().data_ptr(), flux.data_ptr(), _dtype_code(torch, flux), n,
+                                     n_lc, _dp(per), _dp(tt), _dp(dur), float(width), n_masked.data_ptr(),
+                                     ws.data_ptr(), ws.numel(), _stream_ptr(torch, stream))
+    _check(rc, "cetra_mask_transits")
+    return n_masked

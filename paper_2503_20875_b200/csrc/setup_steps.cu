@@ -1,0 +1,363 @@
+// Steps around the two searches: light-curve resampling (§2.1.1, lines 53-61), monotransit
+// search in the linear-search output and transit masking.
+//
+// All of them are HBM-bound streaming kernels (a few bytes of arithmetic per byte moved); every quantity
+// that decides an integer (output point of an observation, in/out of a mask, the exclusion zone of an
+// event) is FP64 with explicitly rounded operations, as in the searches.
+#include <math.h>
+
+#include <algorithm>
+#include <vector>
+
+#include "common.cuh"
+
+namespace cetra {
+
+// ------------------------------------------------------------------------------------------ resample
+// One thread per (light curve, observation): atomically add (w, w f) to the observation's output point.
+template <typename T>
+__global__ void resample_accumulate_kernel(const double *__restrict__ times, const T *__restrict__ flux,
+                                           const T *__restrict__ flux_err, long long n_in, long long n_lc,
+                                           double t_start, double cadence, long long n_out,
+                                           double2 *__restrict__ sums) {
+    const long long total = n_lc * n_in;
+    for (long long idx = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; idx < total;
+         idx += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const long long lc = idx / n_in;
+        const long long i = idx - lc * n_in;
+        const double t = times[i];
+        const double fl = static_cast<double>(flux[idx]);
+        const double er = static_cast<double>(flux_err[idx]);
+        if (!(isfinite(t) && isfinite(fl) && isfinite(er) && er > 0.0)) continue;      // null observation (R8)
+        // nearest output point (R21)
+        const double cell = floor(__dadd_rn(__ddiv_rn(__dsub_rn(t, t_start), cadence), 0.5));
+        if (!(cell >= 0.0 && cell < static_cast<double>(n_out))) continue;
+        const double w = __ddiv_rn(1.0, __dmul_rn(er, er));
+        double2 *dst = sums + lc * n_out + static_cast<long long>(cell);
+        atomicAdd(&dst->x, w);
+        atomicAdd(&dst->y, __dmul_rn(w, fl));
+    }
+}
+
+// One thread per output point: inverse-variance weighted mean and its formal error; null where empty.
+template <typename T>
+__global__ void resample_finalize_kernel(const double2 *__restrict__ sums, long long total, T *__restrict__ flux_out,
+                                         T *__restrict__ err_out) {
+    for (long long idx = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; idx < total;
+         idx += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const double2 s = sums[idx];
+        if (s.x > 0.0) {
+            flux_out[idx] = static_cast<T>(__ddiv_rn(s.y, s.x));
+            err_out[idx] = static_cast<T>(__dsqrt_rn(__ddiv_rn(1.0, s.x)));
+        } else {
+            flux_out[idx] = static_cast<T>(__longlong_as_double(0x7ff8000000000000LL));   // null flux
+            err_out[idx] = static_cast<T>(__longlong_as_double(0x7ff0000000000000LL));    // infinite error
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------- masking
+struct MaskParams {
+    const double *period, *t0, *duration;   // [n_lc] device
+};
+
+template <typename T>
+__global__ void mask_transits_kernel(const double *__restrict__ times, T *__restrict__ flux, long long n,
+                                     long long n_lc, MaskParams mp, double width, int *__restrict__ n_masked) {
+    const long long total = n_lc * n;
+    for (long long idx = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; idx < total;
+         idx += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const long long lc = idx / n;
+        const long long i = idx - lc * n;
+        const double P = mp.period[lc], t0 = mp.t0[lc], D = mp.duration[lc];
+        if (!(isfinite(t0) && D > 0.0)) continue;
+        double d = __dsub_rn(times[i], t0);
+        if (P > 0.0)                                              // distance to the nearest mid-time (R24)
+            d = __dsub_rn(d, __dmul_rn(P, floor(__dadd_rn(__ddiv_rn(d, P), 0.5))));
+        if (fabs(d) <= __dmul_rn(__dmul_rn(0.5, width), D)) {
+            flux[idx] = static_cast<T>(__longlong_as_double(0x7ff8000000000000LL));
+            if (n_masked) atomicAdd(n_masked + lc, 1);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------- monotransit
+// profile(i) = max_j dlogL[j][i], ties -> smallest j; NaN / -1 where every duration is null (R23).
+__global__ void monotransit_profile_kernel(const float *__restrict__ dlogL, long long n_lc, int n_dur,
+                                           long long n_t0, float *__restrict__ prof_lr, int *__restrict__ prof_j) {
+    const long long total = n_lc * n_t0;
+    for (long long idx = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; idx < total;
+         idx += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const long long lc = idx / n_t0;
+        const long long i = idx - lc * n_t0;
+        const float *col = dlogL + lc * n_dur * n_t0 + i;
+        float best = -INFINITY;
+        int bj = -1;
+        for (int j = 0; j < n_dur; ++j) {
+            const float v = col[static_cast<long long>(j) * n_t0];
+            if (v > best || (bj < 0 && v == v)) { best = v; bj = j; }   // NaN compares false; -inf is a value
+        }
+        prof_lr[idx] = bj < 0 ? __int_as_float(0x7fc00000) : best;
+        prof_j[idx] = bj;
+    }
+}
+
+struct EventParams {
+    double durations[CETRA_MAX_DURATIONS];
+};
+
+// One CTA per light curve: n_peaks rounds of (block argmax over the live reference times, record the event,
+// retire its exclusion zone).  Key = (profile bits ordered as unsigned) << 32 | ~i: larger lr, then smaller i.
+__global__ void __launch_bounds__(1024) monotransit_events_kernel(
+    const float *__restrict__ depth, const float *__restrict__ var, const float *__restrict__ prof_lr,
+    const int *__restrict__ prof_j, unsigned char *__restrict__ dead, int n_dur, long long n_t0, double t0_start,
+    double t0_stride, const __grid_constant__ EventParams ep, int n_peaks, double excl,
+    cetra_event *__restrict__ events, int *__restrict__ n_found) {
+    __shared__ unsigned long long s_key[32];
+    __shared__ unsigned long long s_best;
+    const long long lc = blockIdx.x;
+    const float *pl = prof_lr + lc * n_t0;
+    const int *pj = prof_j + lc * n_t0;
+    unsigned char *dd = dead + lc * n_t0;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (long long i = tid; i < n_t0; i += blockDim.x) dd[i] = pj[i] < 0 ? 1 : 0;
+    __syncthreads();
+    int found = 0;
+    for (; found < n_peaks; ++found) {
+        unsigned long long key = 0ull;
+        for (long long i = tid; i < n_t0; i += blockDim.x) {
+            if (dd[i]) continue;
+            const unsigned int b = __float_as_uint(pl[i]);
+            const unsigned int ord = (b & 0x80000000u) ? ~b : (b | 0x80000000u);    // total order of the floats
+            const unsigned long long k = (static_cast<unsigned long long>(ord) << 32) |
+                                         (0xffffffffu - static_cast<unsigned int>(i));
+            key = k > key ? k : key;
+        }
+#pragma unroll
+        for (int s = 16; s > 0; s >>= 1) {
+            const unsigned long long o = __shfl_xor_sync(0xffffffffu, key, s);
+            key = o > key ? o : key;
+        }
+        if (lane == 0) s_key[warp] = key;
+        __syncthreads();
+        if (warp == 0) {
+            key = lane < (blockDim.x >> 5) ? s_key[lane] : 0ull;
+#pragma unroll
+            for (int s = 16; s > 0; s >>= 1) {
+                const unsigned long long o = __shfl_xor_sync(0xffffffffu, key, s);
+                key = o > key ? o : key;
+            }
+            if (lane == 0) s_best = key;
+        }
+        __syncthreads();
+        const unsigned long long best = s_best;
+        if (best == 0ull) break;                                  // no live reference time left
+        const long long bi = 0xffffffffu - static_cast<unsigned int>(best & 0xffffffffull);
+        const int j = pj[bi];
+        if (tid == 0) {
+            cetra_event ev;
+            ev.lr = pl[bi];
+            ev.depth = depth[(lc * n_dur + j) * n_t0 + bi];
+            ev.depth_var = var[(lc * n_dur + j) * n_t0 + bi];
+            ev.t0 = static_cast<float>(__dadd_rn(t0_start, __dmul_rn(static_cast<double>(bi), t0_stride)));
+            ev.i_t0 = static_cast<int>(bi);
+            ev.j_dur = j;
+            ev.reserved[0] = ev.reserved[1] = 0;
+            events[lc * n_peaks + found] = ev;
+        }
+        const double reach = __dmul_rn(excl, ep.durations[j]);
+        for (long long i = tid; i < n_t0; i += blockDim.x)
+            if (i == bi || fabs(__dmul_rn(static_cast<double>(i - bi), t0_stride)) <= reach) dd[i] = 1;
+        __syncthreads();
+    }
+    if (tid == 0) n_found[lc] = found;
+    for (int e = found + tid; e < n_peaks; e += blockDim.x) {
+        cetra_event ev;
+        const float nanv = __int_as_float(0x7fc00000);
+        ev.lr = nanv; ev.depth = nanv; ev.depth_var = nanv; ev.t0 = nanv;
+        ev.i_t0 = -1; ev.j_dur = -1; ev.reserved[0] = ev.reserved[1] = 0;
+        events[lc * n_peaks + e] = ev;
+    }
+}
+
+static int stream_blocks(long long total) {
+    return static_cast<int>(std::max<long long>(1, std::min<long long>((total + 255) / 256, 148LL * 16)));
+}
+
+static bool ws_ok(const void *p, size_t have, size_t need) {
+    return p && (reinterpret_cast<uintptr_t>(p) & (kAlign - 1)) == 0 && have >= need;
+}
+
+static int have_device() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
+        return CETRA_ERR_CUDA;
+    }
+    return CETRA_OK;
+}
+
+}  // namespace cetra
+
+using namespace cetra;
+
+extern "C" {
+
+int cetra_median_cadence(const double *times_host, int64_t n, double *cadence) {
+    if (!times_host || !cadence || n < 2) return CETRA_ERR_INVALID_ARG;
+    std::vector<double> t;
+    t.reserve(static_cast<size_t>(n));
+    for (int64_t i = 0; i < n; ++i)
+        if (std::isfinite(times_host[i])) t.push_back(times_host[i]);
+    if (t.size() < 2) return CETRA_ERR_INVALID_ARG;
+    std::sort(t.begin(), t.end());
+    std::vector<double> d(t.size() - 1);
+    for (size_t i = 0; i + 1 < t.size(); ++i) d[i] = t[i + 1] - t[i];
+    std::sort(d.begin(), d.end());
+    const size_t m = d.size();
+    const double c = (m % 2) ? d[m / 2] : 0.5 * (d[m / 2 - 1] + d[m / 2]);     // R22
+    if (!(c > 0.0)) return CETRA_ERR_INVALID_ARG;
+    *cadence = c;
+    return CETRA_OK;
+}
+
+int cetra_resample_grid(const double *times_host, int64_t n, double cadence, double pad_days, double *t_start,
+                        double *cadence_out, int64_t *n_out) {
+    if (!times_host || !t_start || !cadence_out || !n_out || n < 2 || !(pad_days >= 0.0) || !std::isfinite(pad_days))
+        return CETRA_ERR_INVALID_ARG;
+    double c = cadence;
+    if (!(c > 0.0)) {
+        const int rc = cetra_median_cadence(times_host, n, &c);
+        if (rc != CETRA_OK) return rc;
+    }
+    if (!std::isfinite(c)) return CETRA_ERR_INVALID_ARG;
+    double lo = INFINITY, hi = -INFINITY;
+    for (int64_t i = 0; i < n; ++i) {
+        if (!std::isfinite(times_host[i])) continue;
+        lo = std::min(lo, times_host[i]);
+        hi = std::max(hi, times_host[i]);
+    }
+    if (!(hi >= lo)) return CETRA_ERR_INVALID_ARG;
+    const double pad_n = ceil(pad_days / c);
+    const double span = floor((hi - lo) / c + 0.5) + 1.0 + 2.0 * pad_n;
+    if (!(span < 2.0e9)) return CETRA_ERR_UNSUPPORTED;
+    *t_start = lo - pad_n * c;
+    *cadence_out = c;
+    *n_out = static_cast<int64_t>(span);
+    return CETRA_OK;
+}
+
+size_t cetra_resample_workspace_bytes(int32_t n_lc, int64_t n_out) {
+    if (n_lc < 1 || n_out < 1) return 0;
+    return align_up(sizeof(double2) * static_cast<size_t>(n_lc) * static_cast<size_t>(n_out));
+}
+
+int cetra_resample(const double *times_dev, const void *flux_dev, const void *flux_err_dev, cetra_dtype dtype,
+                   int64_t n_in, int32_t n_lc, double t_start, double cadence, int64_t n_out, void *flux_out_dev,
+                   void *flux_err_out_dev, void *workspace_dev, size_t workspace_bytes, void *cuda_stream) {
+    if (((!times_dev || !flux_dev || !flux_err_dev) && n_in != 0) || !flux_out_dev || !flux_err_out_dev || n_in < 0 ||
+        n_lc < 1 ||
+        n_out < 1 || !(cadence > 0.0) || !std::isfinite(cadence) || !std::isfinite(t_start) ||
+        (dtype != CETRA_F32 && dtype != CETRA_F64))
+        return CETRA_ERR_INVALID_ARG;
+    if (!ws_ok(workspace_dev, workspace_bytes, cetra_resample_workspace_bytes(n_lc, n_out))) return CETRA_ERR_WORKSPACE;
+    if (have_device() != CETRA_OK) return CETRA_ERR_CUDA;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    double2 *sums = static_cast<double2 *>(workspace_dev);
+    const long long total_out = static_cast<long long>(n_lc) * n_out;
+    CETRA_CUDA_TRY(cudaMemsetAsync(sums, 0, sizeof(double2) * static_cast<size_t>(total_out), st));
+    const long long total_in = static_cast<long long>(n_lc) * n_in;
+    if (total_in > 0) {
+        if (dtype == CETRA_F32)
+            resample_accumulate_kernel<float><<<stream_blocks(total_in), 256, 0, st>>>(
+                times_dev, static_cast<const float *>(flux_dev), static_cast<const float *>(flux_err_dev), n_in, n_lc,
+                t_start, cadence, n_out, sums);
+        else
+            resample_accumulate_kernel<double><<<stream_blocks(total_in), 256, 0, st>>>(
+                times_dev, static_cast<const double *>(flux_dev), static_cast<const double *>(flux_err_dev), n_in,
+                n_lc, t_start, cadence, n_out, sums);
+        CETRA_LAUNCH_CHECK();
+    }
+    if (dtype == CETRA_F32)
+        resample_finalize_kernel<float><<<stream_blocks(total_out), 256, 0, st>>>(
+            sums, total_out, static_cast<float *>(flux_out_dev), static_cast<float *>(flux_err_out_dev));
+    else
+        resample_finalize_kernel<double><<<stream_blocks(total_out), 256, 0, st>>>(
+            sums, total_out, static_cast<double *>(flux_out_dev), static_cast<double *>(flux_err_out_dev));
+    CETRA_LAUNCH_CHECK();
+    return CETRA_OK;
+}
+
+size_t cetra_monotransit_workspace_bytes(int32_t n_lc, int64_t n_t0) {
+    if (n_lc < 1 || n_t0 < 1) return 0;
+    const size_t cells = static_cast<size_t>(n_lc) * static_cast<size_t>(n_t0);
+    return align_up(sizeof(float) * cells) + align_up(sizeof(int) * cells) + align_up(cells);
+}
+
+int cetra_monotransit_search(const float *depth_dev, const float *var_dev, const float *dlogL_dev, int32_t n_lc,
+                             int32_t n_dur, cetra_t0_grid grid, const double *durations_host, int32_t n_peaks,
+                             double excl, float *profile_lr_dev, int32_t *profile_j_dev, cetra_event *events_dev,
+                             int32_t *n_found_dev, void *workspace_dev, size_t workspace_bytes, void *cuda_stream) {
+    if (!depth_dev || !var_dev || !dlogL_dev || !durations_host || !events_dev || !n_found_dev || n_lc < 1 ||
+        n_dur < 1 || grid.n_t0 < 1 || n_peaks < 1 || !(excl >= 0.0) || !std::isfinite(excl) ||
+        !(grid.t0_stride > 0.0) || !std::isfinite(grid.t0_stride) || !std::isfinite(grid.t0_start))
+        return CETRA_ERR_INVALID_ARG;
+    if (n_dur > CETRA_MAX_DURATIONS || grid.n_t0 > 0xfffffffeLL) return CETRA_ERR_UNSUPPORTED;
+    EventParams ep;
+    for (int j = 0; j < n_dur; ++j) {
+        if (!(durations_host[j] > 0.0) || !std::isfinite(durations_host[j])) return CETRA_ERR_INVALID_ARG;
+        ep.durations[j] = durations_host[j];
+    }
+    if (!ws_ok(workspace_dev, workspace_bytes, cetra_monotransit_workspace_bytes(n_lc, grid.n_t0)))
+        return CETRA_ERR_WORKSPACE;
+    if (have_device() != CETRA_OK) return CETRA_ERR_CUDA;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    Carver ws(workspace_dev);
+    const size_t cells = static_cast<size_t>(n_lc) * static_cast<size_t>(grid.n_t0);
+    float *pl = ws.take<float>(cells);
+    int *pj = ws.take<int>(cells);
+    unsigned char *dead = ws.take<unsigned char>(cells);
+    if (profile_lr_dev) pl = profile_lr_dev;
+    if (profile_j_dev) pj = profile_j_dev;
+    monotransit_profile_kernel<<<stream_blocks(static_cast<long long>(cells)), 256, 0, st>>>(dlogL_dev, n_lc, n_dur,
+                                                                                            grid.n_t0, pl, pj);
+    CETRA_LAUNCH_CHECK();
+    monotransit_events_kernel<<<n_lc, 1024, 0, st>>>(depth_dev, var_dev, pl, pj, dead, n_dur, grid.n_t0, grid.t0_start,
+                                                     grid.t0_stride, ep, n_peaks, excl, events_dev, n_found_dev);
+    CETRA_LAUNCH_CHECK();
+    return CETRA_OK;
+}
+
+size_t cetra_mask_workspace_bytes(int32_t n_lc) {
+    if (n_lc < 1) return 0;
+    return 3 * align_up(sizeof(double) * static_cast<size_t>(n_lc));
+}
+
+int cetra_mask_transits(const double *times_dev, void *flux_dev, cetra_dtype dtype, int64_t n, int32_t n_lc,
+                        const double *period_host, const double *t0_host, const double *duration_host, double width,
+                        int32_t *n_masked_dev, void *workspace_dev, size_t workspace_bytes, void *cuda_stream) {
+    if (!times_dev || !flux_dev || !period_host || !t0_host || !duration_host || n < 1 || n_lc < 1 ||
+        !(width >= 0.0) || !std::isfinite(width) || (dtype != CETRA_F32 && dtype != CETRA_F64))
+        return CETRA_ERR_INVALID_ARG;
+    if (!ws_ok(workspace_dev, workspace_bytes, cetra_mask_workspace_bytes(n_lc))) return CETRA_ERR_WORKSPACE;
+    if (have_device() != CETRA_OK) return CETRA_ERR_CUDA;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    Carver ws(workspace_dev);
+    double *per = ws.take<double>(n_lc), *t0 = ws.take<double>(n_lc), *dur = ws.take<double>(n_lc);
+    CETRA_CUDA_TRY(cudaMemcpyAsync(per, period_host, sizeof(double) * n_lc, cudaMemcpyHostToDevice, st));
+    CETRA_CUDA_TRY(cudaMemcpyAsync(t0, t0_host, sizeof(double) * n_lc, cudaMemcpyHostToDevice, st));
+    CETRA_CUDA_TRY(cudaMemcpyAsync(dur, duration_host, sizeof(double) * n_lc, cudaMemcpyHostToDevice, st));
+    if (n_masked_dev) CETRA_CUDA_TRY(cudaMemsetAsync(n_masked_dev, 0, sizeof(int32_t) * n_lc, st));
+    MaskParams mp{per, t0, dur};
+    const long long total = static_cast<long long>(n_lc) * n;
+    if (dtype == CETRA_F32)
+        mask_transits_kernel<float><<<stream_blocks(total), 256, 0, st>>>(times_dev, static_cast<float *>(flux_dev), n,
+                                                                          n_lc, mp, width, n_masked_dev);
+    else
+        mask_transits_kernel<double><<<stream_blocks(total), 256, 0, st>>>(times_dev, static_cast<double *>(flux_dev),
+                                                                           n, n_lc, mp, width, n_masked_dev);
+    CETRA_LAUNCH_CHECK();
+    return CETRA_OK;
+}
+
+}  // extern "C"
