@@ -63,6 +63,7 @@ def _load() -> ctypes.CDLL:
         lib.oracle_mask_transits.argtypes = [dp, dp, ctypes.c_int64, ctypes.c_double, ctypes.c_double,
                                              ctypes.c_double, ctypes.c_double, lp]
         lib.oracle_set_threads.argtypes = [ctypes.c_int]
+        lib.oracle_force_general.argtypes = [ctypes.c_int]
         lib.oracle_get_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -105,8 +106,11 @@ class Periodogram:
 
 
 def linear_search(times, flux, flux_err, durations, t0_start: float, t0_stride: float, n_t0: int,
-                  template) -> LinearGrids:
+                  template, force_general: bool = False) -> LinearGrids:
+    """t0 grids on the sample grid use the integer-offset form (R3), others the time-difference form (R25);
+    force_general evaluates an on-grid t0 grid through the R25 form too (a pin of that form)."""
     lib = _load()
+    lib.oracle_force_general(1 if force_general else 0)
     times, flux, flux_err, durations, template = map(_d, (times, flux, flux_err, durations, template))
     n, j = times.shape[0], durations.shape[0]
     depth = np.empty((j, n_t0)); var = np.empty((j, n_t0)); dl = np.empty((j, n_t0))
@@ -114,6 +118,7 @@ def linear_search(times, flux, flux_err, durations, t0_start: float, t0_stride: 
     rc = lib.oracle_linear_search(_p(times, c), _p(flux, c), _p(flux_err, c), n, _p(durations, c), j,
                                   float(t0_start), float(t0_stride), int(n_t0), _p(template, c),
                                   template.shape[0], _p(depth, c), _p(var, c), _p(dl, c))
+    lib.oracle_force_general(0)
     if rc != 0:
         raise ValueError(f"oracle_linear_search failed with status {rc}")
     return LinearGrids(depth, var, dl)

@@ -34,6 +34,10 @@
  *  R10 phases p in [0, ceil(P/s)); R11 epoch cell = p + llrint(e * (P/s)) in FP64.
  *  R12 only durations D_j < P_k, optionally a caller range [dur_lo, dur_hi).
  *  R13 ties: smallest j, then smallest p.
+ *  R25 t0 grids that do not sit on the sample grid (the paper's default stride is 1 % of the shortest
+ *      duration): the nearest-neighbour position is taken from the time difference,
+ *      x = (n*c - (t0_start - times[0] + i*s))/D + 1/2 in FP64, every operation rounded once; grids on
+ *      the sample grid keep the integer-offset form of R3.
  */
 #include <math.h>
 #include <stdint.h>
@@ -48,7 +52,12 @@
 
 static int g_threads = 0;
 
+static int g_force_general = 0;
+
 void oracle_set_threads(int n) { g_threads = n; }
+
+/* Tests only: evaluate grids that sit on the sample grid through the general (R25) form as well. */
+void oracle_force_general(int on) { g_force_general = on; }
 
 int oracle_get_threads(void) {
 #ifdef _OPENMP
@@ -86,9 +95,19 @@ int oracle_linear_search(const double *times, const double *flux, const double *
                          double t0_start, double t0_stride, int64_t n_t0,
                          const double *tpl, int32_t n_tpl,
                          double *depth, double *depth_var, double *dlogL) {
-    double c; int64_t n0, q;
+    double c; int64_t n0 = 0, q = 0;
     int rc = derive_grid(times, n, t0_start, t0_stride, &c, &n0, &q);
-    if (rc) return rc;
+    int general = g_force_general;
+    if (rc == ORACLE_ERR_GRID) {
+        /* regular samples but a t0 grid off the sample grid (R25)?  derive_grid checks the samples first */
+        if (n < 2 || !(t0_stride > 0.0)) return ORACLE_ERR_ARG;
+        c = (times[n - 1] - times[0]) / (double)(n - 1);
+        for (int64_t i = 0; i < n; ++i)
+            if (fabs(times[i] - times[0] - (double)i * c) > 1e-3 * c) return ORACLE_ERR_GRID;
+        general = 1;
+    } else if (rc) {
+        return rc;
+    }
     if (n_dur < 1 || n_t0 < 1 || n_tpl < 2) return ORACLE_ERR_ARG;
     for (int32_t j = 0; j < n_dur; ++j) if (!(durations[j] > 0.0)) return ORACLE_ERR_ARG;
 
@@ -109,10 +128,12 @@ int oracle_linear_search(const double *times, const double *flux, const double *
         const int32_t j = (int32_t)(cell / n_t0);
         const int64_t i = cell % n_t0;
         const double D = durations[j];
+        const int64_t o = (int64_t)j * n_t0 + i;
+        double s_mf = 0.0, s_mm = 0.0, delta = 0.0, ll_model = 0.0, ll_flat = 0.0;
+        if (!general) {
         const int64_t centre = n0 + i * q;                  /* sample index of t_i */
         const int64_t reach = (int64_t)floor(D / (2.0 * c)) + 1;
         /* pass 1: maximum-likelihood depth and its variance */
-        double s_mf = 0.0, s_mm = 0.0;
         for (int64_t k = -reach; k <= reach; ++k) {
             const int64_t nn = centre + k;
             if (nn < 0 || nn >= n) continue;
@@ -122,14 +143,12 @@ int oracle_linear_search(const double *times, const double *flux, const double *
             s_mf += w[nn] * m * f[nn];
             s_mm += w[nn] * m * m;
         }
-        const int64_t o = (int64_t)j * n_t0 + i;
         if (!(s_mm > 0.0)) {                                /* no observation in the window: null */
             depth[o] = NAN; depth_var[o] = NAN; dlogL[o] = NAN;
             continue;
         }
-        const double delta = s_mf / s_mm;
+        delta = s_mf / s_mm;
         /* pass 2: literal Eq. 2 */
-        double ll_model = 0.0, ll_flat = 0.0;
         for (int64_t k = -reach; k <= reach; ++k) {
             const int64_t nn = centre + k;
             if (nn < 0 || nn >= n) continue;
@@ -139,6 +158,33 @@ int oracle_linear_search(const double *times, const double *flux, const double *
             const double r = delta * m - f[nn];
             ll_model += -0.5 * r * r * w[nn];
             ll_flat += -0.5 * f[nn] * f[nn] * w[nn];
+        }
+        } else {
+        /* R25: the reference time relative to the first sample, and a superset of the window's samples */
+        const double ti = (t0_start - times[0]) + (double)i * t0_stride;
+        int64_t lo = (int64_t)floor((ti - 0.5 * D) / c) - 1, hi = (int64_t)floor((ti + 0.5 * D) / c) + 2;
+        if (lo < 0) lo = 0;
+        if (hi > n - 1) hi = n - 1;
+        for (int64_t nn = lo; nn <= hi; ++nn) {
+            const double x = ((double)nn * c - ti) / D + 0.5;
+            if (!(x >= 0.0 && x <= 1.0)) continue;
+            const double m = tpl[(int64_t)floor(x * Mm1 + 0.5)];
+            s_mf += w[nn] * m * f[nn];
+            s_mm += w[nn] * m * m;
+        }
+        if (!(s_mm > 0.0)) {
+            depth[o] = NAN; depth_var[o] = NAN; dlogL[o] = NAN;
+            continue;
+        }
+        delta = s_mf / s_mm;
+        for (int64_t nn = lo; nn <= hi; ++nn) {
+            const double x = ((double)nn * c - ti) / D + 0.5;
+            if (!(x >= 0.0 && x <= 1.0)) continue;
+            const double m = tpl[(int64_t)floor(x * Mm1 + 0.5)];
+            const double r = delta * m - f[nn];
+            ll_model += -0.5 * r * r * w[nn];
+            ll_flat += -0.5 * f[nn] * f[nn] * w[nn];
+        }
         }
         depth[o] = delta;
         depth_var[o] = 1.0 / s_mm;
