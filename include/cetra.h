@@ -24,9 +24,13 @@
  *    CETRA_ERR_NONUNIFORM_TIMES.  Null points (gaps, padding) are marked by a non-finite flux or a
  *    non-finite / non-positive flux_err.  flux is normalised to baseline 1;
  *    internally f = 1 - flux (R7).
- *  - The t0 grid is t_i = t0_start + i*t0_stride, i < n_t0.  t0_start must lie on the
- *    sample grid and t0_stride must be a whole number of cadences (else CETRA_ERR_UNSUPPORTED);
- *    t0_start may lie before times[0] or t_i after times[n-1]: windows are clipped to the data (R9).
+ *  - The t0 grid is t_i = t0_start + i*t0_stride, i < n_t0, any start and any stride > 0.
+ *    When t0_start lies on the sample grid and t0_stride is a whole number of cadences (to 1e-6 cadence)
+ *    the nearest-neighbour template position comes from the integer sample offset (R3) and the fast
+ *    tabulated-tap kernel runs; otherwise (e.g. the paper's default stride, 1 % of the shortest duration)
+ *    it comes from the time difference x = (n*c - (t_i - times[0]))/D + 1/2 in FP64 (R25) and a per-cell
+ *    kernel runs.  t0_start may lie before times[0] or t_i after times[n-1]: windows are clipped to the
+ *    data (R9), which is the paper's null padding expressed through the grid.
  *  - Grids are stored [n_dur][n_t0], t0 contiguous, float32.  Cells whose window holds no
  *    observation are NaN in all three grids.
  *  - Arithmetic: FP32 products and sums on the CUDA cores, FP64 for every
@@ -46,7 +50,7 @@ typedef enum {
     CETRA_OK = 0,
     CETRA_ERR_INVALID_ARG = -1,       /* null pointer, non-positive size, duration <= 0, period < t0_stride ... */
     CETRA_ERR_NONUNIFORM_TIMES = -2,  /* times[] is not a regular grid */
-    CETRA_ERR_UNSUPPORTED = -3,       /* t0 grid off the sample grid, too many durations, index overflow */
+    CETRA_ERR_UNSUPPORTED = -3,       /* too many durations, index overflow */
     CETRA_ERR_WORKSPACE = -4,         /* workspace null, misaligned or smaller than *_workspace_bytes */
     CETRA_ERR_CUDA = -5               /* a CUDA runtime call failed (cudaGetLastError is left set) */
 } cetra_status;

@@ -63,11 +63,12 @@ int derive_geometry(const double *times_host, int64_t n, cetra_t0_grid grid, Geo
     const double b = grid.t0_stride / c;
     if (!(fabs(a) < 1e15) || !(b < 1e15)) return CETRA_ERR_UNSUPPORTED;
     const long long ia = llrint(a), ib = llrint(b);
-    if (fabs(a - static_cast<double>(ia)) > 1e-6 || fabs(b - static_cast<double>(ib)) > 1e-6 || ib < 1)
-        return CETRA_ERR_UNSUPPORTED;
     g->cadence = c;
-    g->n0 = ia;
-    g->q = ib;
+    g->delta = grid.t0_start - times_host[0];
+    g->stride = grid.t0_stride;
+    g->on_grid = !(fabs(a - static_cast<double>(ia)) > 1e-6 || fabs(b - static_cast<double>(ib)) > 1e-6 || ib < 1);
+    g->n0 = g->on_grid ? ia : 0;
+    g->q = g->on_grid ? ib : 0;
     return CETRA_OK;
 }
 

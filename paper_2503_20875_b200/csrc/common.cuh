@@ -50,8 +50,11 @@ struct Carver {
 // Regular-grid geometry shared by the entry points (R1, R9).
 struct Geometry {
     double cadence = 0.0;   // c, days
-    int64_t n0 = 0;         // sample index of t0 cell 0 (may be negative)
-    int64_t q = 0;          // t0 stride in samples (>= 1)
+    bool on_grid = true;    // t0 grid sits on the sample grid with a whole-sample stride (R3), else R25
+    int64_t n0 = 0;         // on_grid: sample index of t0 cell 0 (may be negative)
+    int64_t q = 0;          // on_grid: t0 stride in samples (>= 1)
+    double delta = 0.0;     // t0_start - times[0], days
+    double stride = 0.0;    // t0 stride, days
 };
 
 int derive_geometry(const double *times_host, int64_t n, cetra_t0_grid grid, Geometry *g);

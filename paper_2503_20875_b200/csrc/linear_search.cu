@@ -216,6 +216,55 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
     }
 }
 
+// ------------------------------------------------------------------------------- L2 + L3, off-grid t0
+// The t0 grid does not sit on the sample grid (the paper's default stride is 1 % of the shortest duration,
+// PAPER.md:87), so the template sample of a (cell, sample) pair cannot be tabulated per duration: one thread
+// owns one cell and derives x = (n c - t_i)/D + 1/2 and the nearest-neighbour index per sample in FP64 (R25),
+// exactly rounded operation by operation.  Bound by the FP64 pipe (one IEEE division per template eval);
+// neighbouring lanes read the same samples (the stride is far below the cadence), so loads broadcast.
+__global__ void __launch_bounds__(128) linear_general_kernel(const __grid_constant__ GeneralParams P) {
+    const long long i = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x;
+    const int j = blockIdx.y;
+    const long long lc = blockIdx.z;
+    const long long row = lc * P.n_dur + j;
+    if (i >= P.n_t0) {
+        if (P.stats && i < P.stats_pitch) P.stats[row * P.stats_pitch + i] = make_float2(0.f, 0.f);   // row padding
+        return;
+    }
+    const double D = P.durations[j], c = P.cadence;
+    const double ti = __dadd_rn(P.delta, __dmul_rn(static_cast<double>(i), P.stride));   // t_i - times[0]
+    const double half = __dmul_rn(0.5, D);
+    long long lo = static_cast<long long>(floor(__ddiv_rn(__dsub_rn(ti, half), c))) - 1;  // superset of the window
+    long long hi = static_cast<long long>(floor(__ddiv_rn(__dadd_rn(ti, half), c))) + 2;
+    lo = lo < 0 ? 0 : lo;
+    hi = hi > P.n - 1 ? P.n - 1 : hi;
+    const double Mm1 = static_cast<double>(P.n_tpl - 1);
+    const float2 *x_row = P.wfw + lc * P.lc_pitch;
+    float s_mf = 0.f, s_mm = 0.f;                       // two-level FP32 sums, as in linear_search_kernel
+    for (long long n0 = lo; n0 <= hi; n0 += 64) {
+        float a_mf = 0.f, a_mm = 0.f;
+        const long long n1 = n0 + 63 < hi ? n0 + 63 : hi;
+        for (long long nn = n0; nn <= n1; ++nn) {
+            const double x = __dadd_rn(__ddiv_rn(__dsub_rn(__dmul_rn(static_cast<double>(nn), c), ti), D), 0.5);
+            if (x >= 0.0 && x <= 1.0) {
+                const float m = __ldg(P.tpl + static_cast<int>(floor(__dadd_rn(__dmul_rn(x, Mm1), 0.5))));
+                const float2 s = __ldg(x_row + nn);
+                a_mf = fmaf(m, s.x, a_mf);              // S_wmf += m * (w f)
+                a_mm = fmaf(m * m, s.y, a_mm);          // S_wmm += m^2 * w
+            }
+        }
+        s_mf += a_mf;
+        s_mm += a_mm;
+    }
+    const bool null_cell = !(s_mm > 0.f);               // no observation in the window
+    const float nanv = __int_as_float(0x7fc00000);
+    const float depth = null_cell ? nanv : s_mf / s_mm;
+    if (P.depth) P.depth[row * P.n_t0 + i] = depth;
+    if (P.var) P.var[row * P.n_t0 + i] = null_cell ? nanv : 1.0f / s_mm;
+    if (P.dlogL) P.dlogL[row * P.n_t0 + i] = null_cell ? nanv : 0.5f * s_mf * depth;
+    if (P.stats) P.stats[row * P.stats_pitch + i] = null_cell ? make_float2(0.f, 0.f) : make_float2(s_mm, s_mf);
+}
+
 // ------------------------------------------------------------------------------------------- host
 static size_t linear_smem_bytes(const LinearPlan &pl, int R, int warps) {
     const int tile = warps * 32 * R;
@@ -236,6 +285,23 @@ int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const d
     if (n_dur > CETRA_MAX_DURATIONS) return CETRA_ERR_UNSUPPORTED;
     int rc = derive_geometry(times_host, n, grid, &pl->geo);
     if (rc != CETRA_OK) return rc;
+    if (!pl->geo.on_grid) {
+        // R25: per-cell evaluation; the (w f, w) row is the plain sample array, no tap tables
+        if (n_lc > 65535) return CETRA_ERR_UNSUPPORTED;
+        GeneralParams &G = pl->G;
+        G.n = n; G.n_t0 = grid.n_t0; G.n_dur = n_dur; G.n_tpl = n_template;
+        G.cadence = pl->geo.cadence; G.delta = pl->geo.delta; G.stride = pl->geo.stride;
+        G.lc_pitch = round_up64(n, 4);
+        G.stats_pitch = cetra_stats_pitch(grid.n_t0);
+        for (int j = 0; j < n_dur; ++j) {
+            if (!(durations_host[j] > 0.0) || !std::isfinite(durations_host[j])) return CETRA_ERR_INVALID_ARG;
+            G.durations[j] = durations_host[j];
+        }
+        pl->P.lc_pitch = G.lc_pitch;
+        pl->P.n_lo = 0;
+        pl->taps_total = 0;
+        return CETRA_OK;
+    }
     if (pl->geo.q > (1 << 20)) return CETRA_ERR_UNSUPPORTED;
     LinearParams &P = pl->P;
     constexpr int R = kLinearR;
@@ -334,6 +400,11 @@ int run_linear(LinearPlan &pl, const void *flux_dev, const void *flux_err_dev, c
     P.depth = depth_dev; P.var = var_dev; P.dlogL = dlogL_dev;
     P.stats = reinterpret_cast<float2 *>(stats_dev);
 
+    if (!pl.geo.on_grid && !pl.taps_ready) {
+        CETRA_CUDA_TRY(cudaMemcpyAsync(tpl, template_host, sizeof(float) * n_template,
+                                       template_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+        pl.taps_ready = true;
+    }
     if (!pl.taps_ready) {
         if (template_on_device) {
             CETRA_CUDA_TRY(cudaMemcpyAsync(tpl, template_host, sizeof(float) * n_template, cudaMemcpyDeviceToDevice, st));
@@ -359,6 +430,20 @@ int run_linear(LinearPlan &pl, const void *flux_dev, const void *flux_err_dev, c
                                                              static_cast<const double *>(flux_err_dev), n, n_lc, wfw,
                                                              P.lc_pitch, P.n_lo);
         CETRA_LAUNCH_CHECK();
+    }
+    if (!pl.geo.on_grid) {
+        GeneralParams &G = pl.G;
+        G.wfw = wfw; G.tpl = tpl;
+        G.depth = depth_dev; G.var = var_dev; G.dlogL = dlogL_dev;
+        G.stats = reinterpret_cast<float2 *>(stats_dev);
+        const long long cells = stats_dev ? G.stats_pitch : G.n_t0;
+        const dim3 g(static_cast<unsigned>((cells + 127) / 128), static_cast<unsigned>(G.n_dur),
+                     static_cast<unsigned>(n_lc));
+        profile_mark(kProfLinear, true, st);
+        linear_general_kernel<<<g, 128, 0, st>>>(G);
+        profile_mark(kProfLinear, false, st);
+        CETRA_LAUNCH_CHECK();
+        return CETRA_OK;
     }
     const long long blocks = static_cast<long long>(P.tiles_per_row) * P.n_dur * n_lc;
     constexpr int R = kLinearR;

@@ -22,9 +22,22 @@ struct LinearParams {
     double durations[CETRA_MAX_DURATIONS];
 };
 
+// Off-grid t0 grids (R25): the nearest-neighbour position comes from the time difference, per (cell, sample).
+struct GeneralParams {
+    const float2 *wfw;          // [n_lc][lc_pitch] (w f, w), element 0 is sample 0
+    const float *tpl;           // [n_tpl] device
+    float *depth, *var, *dlogL; // [n_lc][n_dur][n_t0] or null
+    float2 *stats;              // [n_lc][n_dur][stats_pitch] or null
+    long long lc_pitch, n, n_t0, stats_pitch;
+    int n_dur, n_tpl;
+    double cadence, delta, stride;
+    double durations[CETRA_MAX_DURATIONS];
+};
+
 struct LinearPlan {
     Geometry geo;
     LinearParams P{};
+    GeneralParams G{};          // used instead of P when !geo.on_grid
     int warps = 0, tile = 0;
     long long taps_total = 0;
     size_t smem_bytes = 0;

@@ -326,6 +326,56 @@ def test_batched_equals_single_and_host_variant(torch_cuda, cetra, oracle_mod):
         assert_periodic_parity(pk[b], orc, cell, what=f"batch lc {b}")
 
 
+# ------------------------------------------------------------------------------- off-grid t0 grids (R25)
+@pytest.mark.parametrize("cfg,frac", [(1, 0.01), (2, 0.01), (3, 0.037)])
+def test_linear_search_off_grid_t0(cfg, frac, torch_cuda, cetra, oracle_mod):
+    """the default t0 stride is 1 % of the shortest duration, which is not a multiple of the cadence."""
+    p = _problem(cfg)
+    stride = frac * p.durations[0]
+    t0_start = p.times[0] - 0.31 * p.durations[-1]                  # starts before the data: clipped windows
+    n_t0 = {1: 7000, 2: 30000, 3: 6000}[cfg]
+    if cfg == 3:
+        t0_start = p.times[0] + 12.9                                 # runs into the null gap at 13.2 d
+    o = oracle_mod.linear_search(p.times, p.flux, p.flux_err, p.durations, t0_start, stride, n_t0, p.template)
+    flux, err = _dev(torch_cuda, p.flux), _dev(torch_cuda, p.flux_err)
+    r = cetra.cetra_linear_search(p.times, flux, err, p.durations, t0_start, stride, n_t0, p.template, want_stats=True)
+    torch_cuda.cuda.synchronize()
+    worst = assert_linear_parity(r.depth.cpu().numpy(), r.depth_var.cpu().numpy(), r.dlogL.cpu().numpy(),
+                                 o.depth, o.depth_var, o.dlogL, what=f"config {cfg} off-grid")
+    print("off-grid worst", cfg, worst)
+    assert np.isnan(o.depth).any() and (~np.isnan(o.depth)).sum() > 0.5 * o.depth.size
+    # the stats rows hold the same sufficient statistics, zero in null cells and in the padding
+    st = r.stats[0].cpu().numpy()
+    a, b = st[:, :n_t0, 0], st[:, :n_t0, 1]
+    nul = np.isnan(o.depth)
+    assert np.all(a[nul] == 0) and np.all(b[nul] == 0) and np.all(st[:, n_t0:] == 0)
+    assert np.allclose(a[~nul], 1.0 / o.depth_var[~nul], rtol=1e-5)
+
+
+def test_whole_path_off_grid_t0(torch_cuda, cetra, oracle_mod):
+    """Linear + periodic search on the paper's default t0 grid through the batched entry point."""
+    p = _problem(1)
+    stride = 0.01 * p.durations[0]
+    t0_start = p.times[0] - 0.5 * p.durations[-1]                    # PAPER.md:61 padding expressed as a grid start
+    n_t0 = int((p.times[-1] - t0_start + 0.5 * p.durations[-1]) / stride) + 1
+    periods = p.periods[::4]
+    o = oracle_mod.linear_search(p.times, p.flux, p.flux_err, p.durations, t0_start, stride, n_t0, p.template)
+    flux, err = _dev(torch_cuda, p.flux), _dev(torch_cuda, p.flux_err)
+    lin = cetra.cetra_linear_search(p.times, flux, err, p.durations, t0_start, stride, n_t0, p.template)
+    peaks = cetra.peaks_to_numpy(cetra.cetra_search_batched(p.times, flux[None], err[None], p.durations, t0_start,
+                                                            stride, n_t0, p.template, periods))[0]
+    torch_cuda.cuda.synchronize()
+    # periodic parity: the oracle folds the GPU's own linear grids (FP32 -> FP64), as in the on-grid tests
+    import oracle as oracle_pkg
+    g32 = oracle_pkg.LinearGrids(*(a.cpu().numpy().astype(np.float64) for a in (lin.depth, lin.depth_var, lin.dlogL)))
+    orc = oracle_mod.periodic_search(g32, t0_start, stride, p.durations, periods)
+    res = assert_periodic_parity(peaks, orc, lambda k, j, pp: oracle_mod.periodic_cell(g32, stride, periods[k], j, pp),
+                                 what="config 1 off-grid whole path")
+    print("off-grid whole path", res)
+    assert_linear_parity(lin.depth.cpu().numpy(), lin.depth_var.cpu().numpy(), lin.dlogL.cpu().numpy(),
+                         o.depth, o.depth_var, o.dlogL, what="config 1 off-grid grids")
+
+
 # ------------------------------------------------------------------------------- error behaviour
 def test_status_codes_on_device(torch_cuda, cetra):
     p = _problem(1)
@@ -336,7 +386,7 @@ def test_status_codes_on_device(torch_cuda, cetra):
         cetra.cetra_linear_search(bad_times, flux, err, p.durations, p.t0_start, p.t0_stride, p.n_t0, p.template)
     assert e.value.status == cetra.CETRA_ERR_NONUNIFORM_TIMES
     with pytest.raises(cetra.CetraError) as e:
-        cetra.cetra_linear_search(p.times, flux, err, p.durations, p.t0_start, 1.5 * p.cadence, 100, p.template)
+        cetra.cetra_linear_search(p.times, flux, err, np.full(129, 0.05), p.t0_start, p.t0_stride, p.n_t0, p.template)
     assert e.value.status == cetra.CETRA_ERR_UNSUPPORTED
     with pytest.raises(cetra.CetraError) as e:
         cetra.cetra_linear_search(p.times, flux, err, -p.durations, p.t0_start, p.t0_stride, p.n_t0, p.template)
