@@ -385,13 +385,90 @@ def run_survey(args):
     print(json.dumps(line), flush=True)
 
 
+# ------------------------------------------------------------------ BASELINE configs 1-4, stage by stage (optional)
+def run_configs(args):
+    """One JSON line per BASELINE.json config 1-4 (single light curve): linear search and periodic search timed
+    separately with CUDA events (3 warm-ups, median of `--steps` repetitions, L2 flushed in between), as template
+    evaluations/s against the FP32 peak and periods/s + algorithmic GB/s against the HBM and shared-memory peaks;
+    plus the off-grid t0 kernel (paper default stride, 1 % of the shortest duration) and the setup kernels."""
+    import torch
+
+    import paper_2503_20875_b200 as cetra
+    from cetra_synth import make_config, make_irregular_batch
+
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    peaks_hw = measured_peaks()
+    fp32_peak = N_SM * FP32_LANES * 2 * peaks_hw["sm_max_mhz"] * 1e6
+    smem_peak = N_SM * SMEM_BYTES_PER_CLK * peaks_hw["sm_max_mhz"] * 1e6
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+
+    def med_ms(fn, reps):
+        for _ in range(3):
+            fn()
+        out = []
+        for _ in range(reps):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); fn(); b.record()
+            torch.cuda.synchronize()
+            out.append(a.elapsed_time(b))
+        return statistics.median(out)
+
+    for cfg in [int(c) for c in args.cfgs.split(",")]:
+        p = make_config(cfg)
+        wc = work_counts(p)
+        flux, err = torch.from_numpy(p.flux).to(dev), torch.from_numpy(p.flux_err).to(dev)
+        reps = max(1, args.steps if cfg < 4 else min(args.steps, 3))
+        lin_ms = med_ms(lambda: cetra.cetra_linear_search(p.times, flux, err, p.durations, p.t0_start, p.t0_stride,
+                                                          p.n_t0, p.template, want_grids=False, want_stats=True), reps)
+        lin = cetra.cetra_linear_search(p.times, flux, err, p.durations, p.t0_start, p.t0_stride, p.n_t0, p.template,
+                                        want_grids=False, want_stats=True)
+        per_ms = med_ms(lambda: cetra.cetra_periodic_search_stats(lin.stats, p.n_t0, p.t0_start, p.t0_stride,
+                                                                  p.durations, p.periods), reps)
+        fold_bytes = 8.0 * wc["gathers"]
+        line = dict(workload=f"BASELINE configs[{cfg - 1}] {p.name}", n_points=p.n, n_t0=int(p.n_t0),
+                    n_durations=int(len(p.durations)), n_periods=int(len(p.periods)),
+                    linear_ms=lin_ms, template_evals=wc["template_evals"],
+                    template_evals_per_s=wc["template_evals"] / (lin_ms * 1e-3),
+                    linear_frac_fp32=4.0 * wc["template_evals"] / (lin_ms * 1e-3) / fp32_peak,
+                    periodic_ms=per_ms, periods_per_s=len(p.periods) / (per_ms * 1e-3),
+                    fold_algorithmic_gbs=fold_bytes / (per_ms * 1e-3) / 1e9,
+                    fold_frac_hbm=fold_bytes / (per_ms * 1e-3) / 1e9 / peaks_hw["hbm_gbs"],
+                    fold_frac_smem=fold_bytes / (per_ms * 1e-3) / smem_peak,
+                    light_curves_per_s=1e3 / (lin_ms + per_ms), reps=reps,
+                    note="periodic_ms includes finalize_peaks and the key memset; single light curve, so the short "
+                         "configs are launch- and tail-bound")
+        print(json.dumps(line), flush=True)
+        if cfg == 2:
+            stride = 0.01 * p.durations[0]                          # PAPER.md:87 default
+            n_t0 = int((p.times[-1] - p.times[0]) / stride) + 1
+            og_ms = med_ms(lambda: cetra.cetra_linear_search(p.times, flux, err, p.durations, p.times[0], stride, n_t0,
+                                                             p.template, want_grids=False, want_stats=True), reps)
+            evals = wc["template_evals"] * (n_t0 / p.n_t0)
+            print(json.dumps(dict(workload="configs[1] on the paper's default t0 grid (stride = 1 % of the shortest "
+                                           "duration, off the sample grid): linear_general_kernel",
+                                  n_t0=n_t0, linear_ms=og_ms, template_evals_per_s=evals / (og_ms * 1e-3),
+                                  bound="fp64 (one IEEE division per template evaluation)")), flush=True)
+    # setup kernels: resampling 64 irregular light curves of 200 000 observations (HBM-bound streaming)
+    t, f, e = make_irregular_batch(n_lc=64, n=200000)
+    td, fd, ed = (torch.from_numpy(a).to(dev) for a in (t, f, e))
+    t_start, c, n_out = cetra.cetra_resample_grid(t, 0.0, 0.25)
+    rs_ms = med_ms(lambda: cetra.cetra_resample(td, fd, ed, t_start, c, n_out), max(3, args.steps))
+    moved = f.nbytes + e.nbytes + t.nbytes + 64 * n_out * (16 * 2 + 8)       # in + FP64 sums written/read + out
+    print(json.dumps(dict(workload="cetra_resample, 64 curves x %d observations -> %d points" % (t.shape[0], n_out),
+                          ms=rs_ms, algorithmic_gbs=moved / (rs_ms * 1e-3) / 1e9,
+                          frac_hbm=moved / (rs_ms * 1e-3) / 1e9 / peaks_hw["hbm_gbs"])), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--workload", default="sector", choices=["sector", "survey"])
+    ap.add_argument("--workload", default="sector", choices=["sector", "survey", "configs"])
+    ap.add_argument("--cfgs", default="1,2,3,4", help="--workload configs: which BASELINE configs to time")
     ap.add_argument("--n-lc", type=int, default=64, help="light curves per GPU per step (survey: per slice)")
     ap.add_argument("--lc-chunk", type=int, default=0, help="light curves resident at a time (0 = library default)")
     ap.add_argument("--survey-lc", type=int, default=10000)
@@ -406,6 +483,8 @@ def main():
         run_reference(args, rank)
     elif args.workload == "survey":
         run_survey(args)
+    elif args.workload == "configs":
+        run_configs(args)
     else:
         run_cuda(args, rank, world, local_rank)
 
