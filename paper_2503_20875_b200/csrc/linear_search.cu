@@ -6,8 +6,10 @@
 //   L3 (fused epilogue)    depth = S_wmf/S_wmm, var = 1/S_wmm, dlogL = 1/2 S_wmf^2/S_wmm (Eq. 2)
 //
 // The windowed sums are a correlation of the sample stream with 2H_j+1 taps.  For a t0 stride of q
-// samples the taps are split into q polyphase sub-filters, so that R consecutive outputs of one
-// thread slide over a register window: one 8-byte shared-memory load feeds 2R FFMAs.
+// samples both the taps and the samples are split into q polyphase streams (the preprocess kernel
+// writes sample n_lo + q u + v to stream v, position u), so that every branch is a unit-stride
+// correlation in which R consecutive outputs of one thread slide over a register window: one 8-byte
+// shared-memory load feeds 2R FFMAs, and a CTA stages one (tile + taps)-long slice per branch.
 #include "linear_search.cuh"
 
 #include <math.h>
@@ -20,12 +22,17 @@ namespace cetra {
 // ------------------------------------------------------------------------------------------- L0
 template <typename T>
 __global__ void preprocess_kernel(const T *__restrict__ flux, const T *__restrict__ flux_err, long long n,
-                                  long long n_lc, float2 *__restrict__ wfw, long long row_len, long long n_lo) {
+                                  long long n_lc, float2 *__restrict__ wfw, long long ph_pitch, long long q,
+                                  long long n_lo) {
+    // output element (lc, v, u) holds sample n_lo + q u + v: q = 1 is the plain padded sample row
+    const long long row_len = q * ph_pitch;
     const long long total = n_lc * row_len;
     for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
          idx += (long long)gridDim.x * blockDim.x) {
         const long long lc = idx / row_len;
-        const long long nn = idx - lc * row_len + n_lo;
+        const long long e = idx - lc * row_len;
+        const long long v = e / ph_pitch, u = e - v * ph_pitch;
+        const long long nn = n_lo + q * u + v;
         float2 out = make_float2(0.f, 0.f);
         if (nn >= 0 && nn < n) {
             const T fl = flux[lc * n + nn];
@@ -102,7 +109,7 @@ __device__ __forceinline__ float2 add2f(float2 a, float2 b) {
     return r;
 }
 
-template <int R, int WARPS, bool Q1>
+template <int R, int WARPS>
 __global__ void __launch_bounds__(WARPS * 32)
 linear_search_kernel(const __grid_constant__ LinearParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -114,33 +121,41 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
     const int rem = static_cast<int>(blockIdx.x - lc * per_lc);
     const int j = P.order[rem / P.tiles_per_row];               // longest durations first
     const int tile = rem % P.tiles_per_row;
-    const int q = Q1 ? 1 : P.q;
+    const int q = P.q;
     const int A = P.A[j];
     const long long i_blk = static_cast<long long>(tile) * TILE;
-
-    // sample range of this tile in the padded (w f, w) row: starts at the first tap of the first output
-    const long long s_first = P.n0 - P.H[j] + q * i_blk - P.n_lo;
-    const int d0 = static_cast<int>(s_first & 1);                // bulk copies need 16-byte alignment
-    const int len = (d0 + q * (TILE + A) + 1) & ~1;
     const int n_tap = P.tap_off[j + 1] - P.tap_off[j];
+    const int slice = (TILE + A + 2) & ~1;                       // samples of one branch (+ alignment slack)
 
-    uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
-    float2 *data = reinterpret_cast<float2 *>(smem_raw + 16);
-    float2 *taps = data + len;
-    float2 *stage = taps + n_tap;
+    // element of the first tap of output 0 in the padded sample numbering; branch b starts b samples later
+    const unsigned int e0 = static_cast<unsigned int>(P.n0 - P.H[j] - P.n_lo);   // <= h_max + 2, far below 2^31
+    const unsigned int uq = static_cast<unsigned int>(q);
+
+    uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);      // bar[0], bar[1]: one per sample stage
+    float2 *taps = reinterpret_cast<float2 *>(smem_raw + 32);
+    float2 *stage0 = taps + n_tap;                               // two sample stages of `slice` elements
+
+    // branch b reads stream v = (e0 + b) mod q from position (e0 + b) div q + i_blk on
+    auto issue = [&](int b, bool with_taps) {
+        const unsigned int e = e0 + static_cast<unsigned int>(b);
+        const long long v = e % uq, u0 = e / uq + i_blk;
+        const int d0 = static_cast<int>(u0 & 1);                 // bulk copies need 16-byte alignment
+        const uint32_t bytes = static_cast<uint32_t>(slice) * 8u;
+        const uint32_t bytes_taps = with_taps ? static_cast<uint32_t>(n_tap) * 8u : 0u;
+        uint64_t *bb = bar + (b & 1);
+        if (b > 1) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the stage was read by generic loads
+        mbar_arrive_expect_tx(bb, bytes + bytes_taps);
+        bulk_copy_g2s_chunked(stage0 + (b & 1) * slice, P.wfw + (lc * q + v) * P.ph_pitch + (u0 - d0), bytes, bb);
+        if (with_taps) bulk_copy_g2s_chunked(taps, P.taps + P.tap_off[j], bytes_taps, bb);
+    };
 
     if (tid == 0) {
         mbar_init(bar, 1);
+        if (q > 1) mbar_init(bar + 1, 1);
         mbar_fence_init();
+        issue(0, true);
     }
     __syncthreads();
-    if (tid == 0) {
-        const uint32_t bytes_data = static_cast<uint32_t>(len) * 8u, bytes_taps = static_cast<uint32_t>(n_tap) * 8u;
-        mbar_arrive_expect_tx(bar, bytes_data + bytes_taps);
-        bulk_copy_g2s_chunked(data, P.wfw + lc * P.lc_pitch + (s_first - d0), bytes_data, bar);
-        bulk_copy_g2s_chunked(taps, P.taps + P.tap_off[j], bytes_taps, bar);
-    }
-    mbar_wait(bar, 0);
 
     // Two-level summation: the running FFMA accumulators are folded into a second set every kFlush tap
     // groups (and at the end of every polyphase branch), so that no FP32 sum runs over more than
@@ -151,24 +166,25 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
 #pragma unroll
     for (int r = 0; r < R; ++r) { acc[r] = make_float2(0.f, 0.f); tot[r] = make_float2(0.f, 0.f); }
 
-    const float2 *xs = data + d0 + q * (tid * R);
     for (int b = 0; b < q; ++b) {
-        const float2 *xb = xs + b;
+        if (tid == 0 && b + 1 < q) issue(b + 1, false);          // its stage was released at the end of branch b-1
+        mbar_wait(bar + (b & 1), static_cast<uint32_t>((b >> 1) & 1));
+        const int d0 = static_cast<int>(((e0 + static_cast<unsigned int>(b)) / uq + i_blk) & 1);
+        const float2 *xb = stage0 + (b & 1) * slice + d0 + tid * R;
         const float2 *tb = taps + b * A;
         float2 win[R];
 #pragma unroll
-        for (int v = 0; v < R - 1; ++v) win[v] = xb[q * v];
-        float2 nxt = xb[q * (R - 1)];
+        for (int v = 0; v < R - 1; ++v) win[v] = xb[v];
+        float2 nxt = xb[R - 1];
         float2 tap = tb[0];
-        const float2 *xp = xb + q * R;
+        const float2 *xp = xb + R;
         int since_flush = 0;
         for (int a0 = 0; a0 < A; a0 += R) {
 #pragma unroll
             for (int u = 0; u < R; ++u) {
                 win[(u + R - 1) % R] = nxt;
                 const float2 t = tap;
-                nxt = Q1 ? xp[u] : *xp;                          // prefetch the next window element
-                if (!Q1) xp += q;
+                nxt = xp[u];                                     // prefetch the next window element
                 tap = tb[a0 + u + 1];
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
@@ -176,7 +192,7 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
                     acc[r] = fma2(t, win[(u + r) % R], acc[r]);
                 }
             }
-            if (Q1) xp += R;
+            xp += R;
             if (++since_flush == kFlush || a0 + R >= A) {
                 since_flush = 0;
 #pragma unroll
@@ -186,7 +202,10 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
                 }
             }
         }
+        if (q > 1) __syncthreads();                              // every warp is done with this stage
     }
+    // transposition buffer of the epilogue: the consumed stages when there were several branches, else its own
+    float2 *stage = q > 1 ? stage0 : stage0 + slice;
 
     // transpose through shared memory so that the global stores are coalesced
     float2 *st = stage + warp * (32 * R);
@@ -267,12 +286,14 @@ __global__ void __launch_bounds__(128) linear_general_kernel(const __grid_consta
 
 // ------------------------------------------------------------------------------------------- host
 static size_t linear_smem_bytes(const LinearPlan &pl, int R, int warps) {
+    // barriers, the duration's tap table (all branches), then either two sample stages (several branches; the
+    // epilogue's transposition buffer aliases them) or one stage and the transposition buffer (one branch)
     const int tile = warps * 32 * R;
     size_t worst = 0;
     for (int j = 0; j < pl.P.n_dur; ++j) {
-        const size_t len = (static_cast<size_t>(1 + pl.P.q * (tile + pl.P.A[j]) + 1)) & ~size_t(1);
+        const size_t slice = (static_cast<size_t>(tile + pl.P.A[j] + 2)) & ~size_t(1);
         const size_t n_tap = pl.P.tap_off[j + 1] - pl.P.tap_off[j];
-        worst = std::max(worst, 16 + (len + n_tap + tile) * 8);
+        worst = std::max(worst, 32 + (n_tap + (pl.P.q > 1 ? 2 * slice : slice + tile)) * 8);
     }
     return worst;
 }
@@ -335,6 +356,7 @@ int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const d
     for (int j = 0; j < n_dur; ++j) P.order[j] = static_cast<unsigned char>(ord[j]);
 
     // tile shape: as many warps per block as shared memory allows, fewer when the grid would not fill the chip
+    // (picking the width that wastes the fewest cells in a row's last tile measured slower: 0.496 vs 0.465 ms)
     int warps = 4;
     for (;;) {
         const int tile = warps * 32 * R;
@@ -353,10 +375,11 @@ int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const d
     if (static_cast<long long>(P.tiles_per_row) * n_dur * n_lc > 0x7fffffffLL) return CETRA_ERR_UNSUPPORTED;
     pl->smem_bytes = linear_smem_bytes(*pl, R, warps);
 
-    // padded (w f, w) row: sample index n_lo is element 0
+    // padded (w f, w) samples in q polyphase streams: element u of stream v is sample n_lo + q u + v
     P.n_lo = P.n0 - h_max - 2;
-    const long long n_hi = P.n0 + static_cast<long long>(P.q) * (static_cast<long long>(P.tiles_per_row) * pl->tile + a_max) + P.q + 4;
-    P.lc_pitch = round_up64(n_hi - P.n_lo, 4);
+    const long long u_hi = (h_max + 2 + P.q) / P.q + static_cast<long long>(P.tiles_per_row) * pl->tile + a_max + 8;
+    P.ph_pitch = round_up64(u_hi, 4);
+    P.lc_pitch = P.ph_pitch * P.q;
     P.stats_pitch = cetra_stats_pitch(grid.n_t0);
     return CETRA_OK;
 }
@@ -371,15 +394,9 @@ size_t linear_workspace_bytes(const LinearPlan &pl, int32_t n_lc, int32_t n_temp
 
 template <int R, int WARPS>
 static int launch_linear(const LinearPlan &pl, const LinearParams &P, long long blocks, cudaStream_t st) {
-    if (P.q == 1) {
-        auto k = linear_search_kernel<R, WARPS, true>;
-        CETRA_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes));
-        k<<<static_cast<unsigned>(blocks), WARPS * 32, pl.smem_bytes, st>>>(P);
-    } else {
-        auto k = linear_search_kernel<R, WARPS, false>;
-        CETRA_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes));
-        k<<<static_cast<unsigned>(blocks), WARPS * 32, pl.smem_bytes, st>>>(P);
-    }
+    auto k = linear_search_kernel<R, WARPS>;
+    CETRA_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes));
+    k<<<static_cast<unsigned>(blocks), WARPS * 32, pl.smem_bytes, st>>>(P);
     CETRA_LAUNCH_CHECK();
     return CETRA_OK;
 }
@@ -420,15 +437,17 @@ int run_linear(LinearPlan &pl, const void *flux_dev, const void *flux_err_dev, c
     }
     {
         const long long total = static_cast<long long>(n_lc) * P.lc_pitch;
+        // off-grid plans keep the plain sample row (one stream)
+        const long long ph_q = pl.geo.on_grid ? P.q : 1, ph_pitch = pl.geo.on_grid ? P.ph_pitch : P.lc_pitch;
         const int blocks = static_cast<int>(std::min<long long>((total + 255) / 256, 148LL * 16));
         if (dtype == CETRA_F32)
             preprocess_kernel<float><<<blocks, 256, 0, st>>>(static_cast<const float *>(flux_dev),
                                                             static_cast<const float *>(flux_err_dev), n, n_lc, wfw,
-                                                            P.lc_pitch, P.n_lo);
+                                                            ph_pitch, ph_q, P.n_lo);
         else
             preprocess_kernel<double><<<blocks, 256, 0, st>>>(static_cast<const double *>(flux_dev),
                                                              static_cast<const double *>(flux_err_dev), n, n_lc, wfw,
-                                                             P.lc_pitch, P.n_lo);
+                                                             ph_pitch, ph_q, P.n_lo);
         CETRA_LAUNCH_CHECK();
     }
     if (!pl.geo.on_grid) {

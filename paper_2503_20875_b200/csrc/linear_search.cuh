@@ -9,11 +9,11 @@ constexpr int kLinearR = 15;   // consecutive t0 cells per thread; odd => confli
 
 // Passed by value (__grid_constant__): no device copy, no host synchronisation.
 struct LinearParams {
-    const float2 *wfw;          // [n_lc][lc_pitch] (w f, w), element 0 is sample index n_lo
+    const float2 *wfw;          // [n_lc][q][ph_pitch] (w f, w): element u of stream v is sample n_lo + q u + v
     const float2 *taps;         // per duration [q][A_j] (m, m^2), see build_taps_kernel
     float *depth, *var, *dlogL; // [n_lc][n_dur][n_t0] or null
     float2 *stats;              // [n_lc][n_dur][stats_pitch] or null
-    long long lc_pitch, n_lo, n0, n_t0, stats_pitch;
+    long long lc_pitch, ph_pitch, n_lo, n0, n_t0, stats_pitch;   // lc_pitch = q * ph_pitch elements per light curve
     int q, n_dur, tiles_per_row;
     int H[CETRA_MAX_DURATIONS];         // window half-reach in samples (superset of the window)
     int A[CETRA_MAX_DURATIONS];         // taps per polyphase branch, padded to a multiple of kLinearR
