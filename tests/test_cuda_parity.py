@@ -326,6 +326,45 @@ def test_batched_equals_single_and_host_variant(torch_cuda, cetra, oracle_mod):
         assert_periodic_parity(pk[b], orc, cell, what=f"batch lc {b}")
 
 
+def test_bench_configuration_sampled_against_oracle(torch_cuda, cetra, oracle_mod):
+    """The launch configuration bench.py times: 64 survey curves of BASELINE configs[1] in one chunk, all 20 000
+    periods.  Records of sampled (curve, period) pairs are checked against the oracle one by one, and properties
+    that hold at any size on all 1.28 million records."""
+    from cetra_synth import make_survey_batch
+    p = make_survey_batch(n_lc=64, lc_range=(0, 64))
+    flux, err = _dev(torch_cuda, p.flux), _dev(torch_cuda, p.flux_err)
+    pk = cetra.peaks_to_numpy(cetra.cetra_search_batched(p.times, flux, err, p.durations, p.t0_start, p.t0_stride,
+                                                         p.n_t0, p.template, p.periods))
+    K = p.periods.shape[0]
+    assert pk.shape == (64, K)
+    # properties of every record (PAPER.md:145, R10, R13)
+    ok = pk["i_t0"] >= 0
+    assert ok.all()                                          # every period has a candidate in these curves
+    assert np.all(pk["lr"] >= 0) and np.all(pk["depth_var"] > 0) and np.all(pk["n_transits"] >= 1)
+    assert np.all(p.durations[pk["j_dur"]] < p.periods[None, :])
+    assert np.all(pk["i_t0"] < np.ceil(p.periods / p.t0_stride)[None, :])
+    n_epochs_max = np.floor((p.n_t0 - 1) / (p.periods / p.t0_stride)) + 1
+    assert np.all(pk["n_transits"] <= n_epochs_max[None, :] + 1)
+    assert np.allclose(pk["lr"], 0.5 * pk["depth"].astype(np.float64) ** 2 / pk["depth_var"], rtol=1e-5)
+    rng = np.random.default_rng(64)
+    injected = [b for b, i in enumerate(p.injections) if i["period"] is not None]
+    for b in (injected[0], injected[-1], [b for b in range(64) if b not in injected][0]):
+        sel = set(rng.choice(K, 30, replace=False).tolist()) | {int(np.argmax(pk[b]["lr"]))}
+        if p.injections[b]["period"] is not None:
+            k_inj = int(np.argmin(np.abs(p.periods - p.injections[b]["period"])))
+            sel |= set(range(max(0, k_inj - 3), min(K, k_inj + 4)))
+        sel = np.array(sorted(sel))
+        o = oracle_mod.linear_search(p.times, p.flux[b], p.flux_err[b], p.durations, p.t0_start, p.t0_stride,
+                                     p.n_t0, p.template)
+        orc = oracle_mod.periodic_search(o, p.t0_start, p.t0_stride, p.durations, p.periods[sel])
+
+        def cell(k, j, ph):
+            return oracle_mod.periodic_cell(o, p.t0_stride, p.periods[sel][k], j, ph)
+
+        res = assert_periodic_parity(pk[b][sel], orc, cell, what=f"bench configuration, curve {b}")
+        print("bench configuration curve", b, res)
+
+
 # ------------------------------------------------------------------------------- off-grid t0 grids (R25)
 @pytest.mark.parametrize("cfg,frac", [(1, 0.01), (2, 0.01), (3, 0.037)])
 def test_linear_search_off_grid_t0(cfg, frac, torch_cuda, cetra, oracle_mod):
