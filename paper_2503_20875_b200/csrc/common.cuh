@@ -28,7 +28,7 @@ extern std::atomic<int64_t> g_launch_count;
 enum ProfiledKernel { kProfLinear = 0, kProfFold = 1 };
 void profile_mark(ProfiledKernel which, bool begin, cudaStream_t st);
 
-constexpr int kStatsPad = 128;          // zero cells after the last t0 cell of every stats row
+constexpr int kStatsPad = 512;          // zero cells after the last t0 cell of every stats row
 constexpr size_t kAlign = 256;          // workspace carve-up alignment
 
 inline size_t align_up(size_t x, size_t a = kAlign) { return (x + a - 1) / a * a; }

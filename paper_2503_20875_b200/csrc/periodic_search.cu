@@ -225,6 +225,245 @@ __global__ void __launch_bounds__(kFoldThreads, 1) fold_argmax_kernel(const __gr
     }
 }
 
+// ------------------------------------------------------------------------------- grouped fold (P1-P4)
+// Neighbouring trial periods fold almost the same cells: at epoch e the offsets llrint(e r_k) of kGrpT
+// consecutive periods differ by a few cells.  A warp therefore folds kGrpT periods together; a lane owns
+// G consecutive phases and, per epoch, loads the G + d_max cells that cover all kGrpT periods into a
+// register window once (8-byte LDS at a lane stride of G cells: G odd => conflict-free) and adds them into
+// the kGrpT x G accumulators at the period's shift d_t = off_t(e) - off_0(e), a warp-uniform switch.  One
+// load then feeds up to kGrpT adds, which lifts the kernel off the shared-memory crossbar (the per-period
+// kernel's limit, profiles/r01c).  The per-cell arithmetic, the order of the epoch sum and the offsets
+// (FP64, R11) are exactly those of the per-period kernel.  Epochs whose offsets spread over more than
+// kGrpS cells (long periods) are gathered period by period in the same loop.
+template <int D, int G, int W>
+__device__ __forceinline__ void add_window(float2 (&acc)[G], const float2 (&c)[W]) {
+#pragma unroll
+    for (int g = 0; g < G; ++g) acc[g] = add2(acc[g], c[g + D]);
+}
+
+template <int G, int W>
+__device__ __forceinline__ void add_shifted(float2 (&acc)[G], const float2 (&c)[W], int d) {
+    static_assert(W == G + kGrpS && kGrpS == 7, "one case per shift");
+    switch (d) {
+        case 0: add_window<0, G, W>(acc, c); break;
+        case 1: add_window<1, G, W>(acc, c); break;
+        case 2: add_window<2, G, W>(acc, c); break;
+        case 3: add_window<3, G, W>(acc, c); break;
+        case 4: add_window<4, G, W>(acc, c); break;
+        case 5: add_window<5, G, W>(acc, c); break;
+        case 6: add_window<6, G, W>(acc, c); break;
+        default: add_window<7, G, W>(acc, c); break;
+    }
+}
+
+struct GroupPeriods {
+    double r[kGrpT];          // period in t0 cells, ascending
+    int n_phase[kGrpT];       // R10; 0 for a period that is not searched on this row
+};
+
+__device__ __forceinline__ float2 lds_cell(uint32_t addr) {
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+    return v;
+}
+
+// One pass of a warp over 32*G consecutive phases starting at p0; lane owns phases p0 + lane*G + g.
+// ew: the warp's shared-memory slots for one block of 32 epochs: ew[e] = (off_0, off_1), the offsets of the two
+// periods of the group (off_1 >= off_0 because the periods are sorted).  When off_1 - off_0 <= kGrpS the G + d
+// cells from off_0 on serve both periods from one register window; otherwise each period gathers its own cells.
+template <int G, bool kLastPass>
+__device__ __forceinline__ void fold_group_pass(uint32_t srow, int p0, int n_t0, const GroupPeriods &gp,
+                                                int2 *__restrict__ ew, int lane, float (&best_lr)[kGrpT],
+                                                int (&best_p)[kGrpT]) {
+    static_assert(kGrpT == 2, "two periods per warp");
+    constexpr int W = G + kGrpS;
+    float2 acc[kGrpT][G];
+    float2 c[W];
+#pragma unroll
+    for (int t = 0; t < kGrpT; ++t)
+#pragma unroll
+        for (int g = 0; g < G; ++g) acc[t][g] = make_float2(0.f, 0.f);
+#pragma unroll
+    for (int i = 0; i < W; ++i) c[i] = make_float2(0.f, 0.f);
+    const long long limit = static_cast<long long>(n_t0) - 1 - p0;   // off_e <= limit  <=>  p0 + off_e <= I-1
+    const uint32_t base = srow + 8u * static_cast<uint32_t>(p0 + lane * G);
+    for (int eb = 0;; eb += 32) {
+        // P1: lane l derives the offsets of epoch eb + l for the two periods (FP64, R11)
+        const double e = static_cast<double>(eb + lane);
+        const long long o0 = __double2ll_rn(__dmul_rn(e, gp.r[0]));
+        const long long o1 = __double2ll_rn(__dmul_rn(e, gp.r[1]));
+        const bool ok = o0 <= limit;                                  // r ascending: o0 is the smaller
+        const long long cap = 0x0fffffffLL;
+        __syncwarp();                                                 // the previous block's words are consumed
+        ew[lane] = make_int2(static_cast<int>(o0 < cap ? o0 : cap), static_cast<int>(o1 < cap ? o1 : cap));
+        __syncwarp();
+        const int cnt = __popc(__ballot_sync(0xffffffffu, ok));       // offsets are monotone in e: a prefix is valid
+        for (int t = 0; t < cnt; ++t) {
+            const int2 w = ew[t];                                     // broadcast load
+            const uint32_t ptr = base + 8u * static_cast<uint32_t>(w.x);
+            const int d = w.y - w.x;
+            if (d <= kGrpS) {
+#pragma unroll
+                for (int i = 0; i < G; ++i) c[i] = lds_cell(ptr + 8u * i);
+#pragma unroll
+                for (int i = G; i < W; ++i)
+                    if (i < G + d) c[i] = lds_cell(ptr + 8u * i);
+                add_window<0, G, W>(acc[0], c);
+                add_shifted<G, W>(acc[1], c, d);
+            } else {
+#pragma unroll
+                for (int g = 0; g < G; ++g) acc[0][g] = add2(acc[0][g], lds_cell(ptr + 8u * g));
+                if (w.y <= limit) {
+                    const uint32_t pu = base + 8u * static_cast<uint32_t>(w.y);
+#pragma unroll
+                    for (int g = 0; g < G; ++g) acc[1][g] = add2(acc[1][g], lds_cell(pu + 8u * g));
+                }
+            }
+        }
+        if (cnt < 32) break;
+    }
+    // P3 + P4 within the lane: phases ascending, strict > keeps the smallest phase on ties.  A cell with no
+    // contributing epoch has S_wmm = 0 (and S_wmf = 0): it is not a candidate.
+#pragma unroll
+    for (int t = 0; t < kGrpT; ++t) {
+#pragma unroll
+        for (int g = 0; g < G; ++g) {
+            const int p = p0 + lane * G + g;
+            const float a = acc[t][g].x, bsum = acc[t][g].y;
+            const float lr = 0.5f * bsum * bsum * rcp_approx(a);
+            const bool in = kLastPass ? p < gp.n_phase[t] : true;
+            if (in && a > 0.f && lr > best_lr[t]) { best_lr[t] = lr; best_p[t] = p; }
+        }
+    }
+}
+
+__global__ void __launch_bounds__(kGrpThreads, 1) fold_group_argmax_kernel(const __grid_constant__ PeriodicParams P) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    constexpr int kWarps = kGrpThreads / 32;
+    constexpr int kUnitPeriods = kWarps * kGrpT;
+    uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
+    unsigned int *s_claim = reinterpret_cast<unsigned int *>(smem_raw + 8);
+    int2 *s_ew = reinterpret_cast<int2 *>(smem_raw + 16);                              // [kWarps][32]
+    float2 *srow = reinterpret_cast<float2 *>(smem_raw + kGrpHeaderBytes);
+    const uint32_t srow_addr = smem_u32(srow);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    int2 *ew = s_ew + warp * 32;
+
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    long long cur_row = -1;
+    uint32_t parity = 0;
+    for (;;) {
+        if (tid == 0) {
+            const long long seen = *reinterpret_cast<volatile unsigned int *>(P.counter);   // may be stale: only sizes the claim
+            long long want = (P.n_units - seen) / (2LL * gridDim.x);
+            want = want < 1 ? 1 : (want > P.max_claim ? P.max_claim : want);
+            s_claim[0] = atomicAdd(P.counter, static_cast<unsigned int>(want));
+            s_claim[1] = static_cast<unsigned int>(want);
+        }
+        __syncthreads();
+        long long u = s_claim[0];
+        const long long u_end = min(u + static_cast<long long>(s_claim[1]), P.n_units);
+        __syncthreads();                       // everyone has read the slot and is done with the previous claim
+        if (u >= P.n_units) break;
+        while (u < u_end) {
+            const long long rowid = u / P.units_per_row;               // lc * n_dur + j
+            const long long u_row0 = rowid * P.units_per_row;
+            const long long u_stop = min(u_end, u_row0 + P.units_per_row);
+            const int j = static_cast<int>(rowid % P.n_dur);
+            const long long lc = rowid / P.n_dur;
+            if (rowid != cur_row) {
+                __syncthreads();               // every warp is done with the row about to be overwritten
+                if (tid == 0) {
+                    const uint32_t bytes = static_cast<uint32_t>(P.stats_pitch) * 8u;
+                    mbar_arrive_expect_tx(bar, bytes);
+                    bulk_copy_g2s_chunked(srow, P.stats + rowid * P.stats_pitch, bytes, bar);
+                }
+                mbar_wait(bar, parity);
+                parity ^= 1u;
+                cur_row = rowid;
+            }
+            const double D = P.durations[j];
+            const int k_end = static_cast<int>(min(static_cast<long long>(P.n_per), (u_stop - u_row0) * kUnitPeriods));
+            for (int k0 = static_cast<int>(u - u_row0) * kUnitPeriods + warp * kGrpT; k0 < k_end;
+                 k0 += kUnitPeriods) {
+                // the group's periods, sorted by ascending r (warp-uniform values)
+                GroupPeriods gp;
+                int kk[kGrpT];
+                int n_phase_max = 0;
+#pragma unroll
+                for (int t = 0; t < kGrpT; ++t) {
+                    const int k = min(k0 + t, P.n_per - 1);            // ragged last group: repeat the last period
+                    const double period = P.periods[k];
+                    bool on = k0 + t < P.n_per && D < period;          // overlapping windows are invalid
+                    if (on && P.dur_lo && (j < P.dur_lo[k] || j >= P.dur_hi[k])) on = false;
+                    const double r = __ddiv_rn(period, P.t0_stride);   // period in t0 cells, FP64 (R11)
+                    const double rc = ceil(r);
+                    const int n_phase = rc < static_cast<double>(P.n_t0) ? static_cast<int>(rc) : P.n_t0;   // R10
+                    gp.r[t] = r;
+                    gp.n_phase[t] = on ? n_phase : 0;
+                    kk[t] = k;
+                    n_phase_max = max(n_phase_max, gp.n_phase[t]);
+                }
+                if (n_phase_max == 0) continue;
+#define CETRA_CSWAP(a, b)                                                                         \
+    if (gp.r[a] > gp.r[b]) {                                                                      \
+        const double tr = gp.r[a]; gp.r[a] = gp.r[b]; gp.r[b] = tr;                               \
+        const int tn = gp.n_phase[a]; gp.n_phase[a] = gp.n_phase[b]; gp.n_phase[b] = tn;          \
+        const int tk = kk[a]; kk[a] = kk[b]; kk[b] = tk;                                          \
+    }
+                CETRA_CSWAP(0, 1)
+#undef CETRA_CSWAP
+                int n_phase_min = 0x7fffffff;                          // over the searched periods of the group
+#pragma unroll
+                for (int t = 0; t < kGrpT; ++t)
+                    if (gp.n_phase[t] > 0) n_phase_min = min(n_phase_min, gp.n_phase[t]);
+                const bool all_on = gp.n_phase[0] > 0 && gp.n_phase[1] > 0;
+                float best_lr[kGrpT];
+                int best_p[kGrpT];
+#pragma unroll
+                for (int t = 0; t < kGrpT; ++t) { best_lr[t] = -1.f; best_p[t] = 0x7fffffff; }
+                // full passes while every phase of the pass is a phase of every period of the group
+                int p0 = 0;
+                if (all_on)
+                    for (; p0 + 32 * kGrpG <= n_phase_min; p0 += 32 * kGrpG)
+                        fold_group_pass<kGrpG, false>(srow_addr, p0, P.n_t0, gp, ew, lane, best_lr, best_p);
+                for (; p0 + 32 * kGrpG < n_phase_max; p0 += 32 * kGrpG)
+                    fold_group_pass<kGrpG, true>(srow_addr, p0, P.n_t0, gp, ew, lane, best_lr, best_p);
+                // the last pass: the narrowest of G = 1, 3, 7, kGrpG phases per lane that covers what is left
+                const int left = n_phase_max - p0;
+                if (left > 32 * 7) fold_group_pass<kGrpG, true>(srow_addr, p0, P.n_t0, gp, ew, lane, best_lr, best_p);
+                else if (left > 32 * 3) fold_group_pass<7, true>(srow_addr, p0, P.n_t0, gp, ew, lane, best_lr, best_p);
+                else if (left > 32) fold_group_pass<3, true>(srow_addr, p0, P.n_t0, gp, ew, lane, best_lr, best_p);
+                else if (left > 0) fold_group_pass<1, true>(srow_addr, p0, P.n_t0, gp, ew, lane, best_lr, best_p);
+                // P4 across the warp: larger lr wins, ties -> smaller phase; one atomicMax per period
+#pragma unroll
+                for (int t = 0; t < kGrpT; ++t) {
+                    float lr = best_lr[t];
+                    int p = best_p[t];
+#pragma unroll
+                    for (int s = 16; s > 0; s >>= 1) {
+                        const float o_lr = __shfl_xor_sync(0xffffffffu, lr, s);
+                        const int o_p = __shfl_xor_sync(0xffffffffu, p, s);
+                        if (o_lr > lr || (o_lr == lr && o_p < p)) { lr = o_lr; p = o_p; }
+                    }
+                    if (lane == 0 && lr >= 0.f) {
+                        const unsigned int id = static_cast<unsigned int>(j) * static_cast<unsigned int>(P.n_t0) +
+                                                static_cast<unsigned int>(p);
+                        const unsigned long long key =
+                            (static_cast<unsigned long long>(__float_as_uint(lr)) << 32) | (0xffffffffu - id);
+                        atomicMax(P.keys + lc * P.n_per + kk[t], key);
+                    }
+                }
+            }
+            u = u_stop;
+        }
+    }
+}
+
 // One thread per (light curve, period): decode the winning (j, p), redo its fold in the same order with
 // IEEE division, count the contributing epochs and write the record.
 __global__ void finalize_peaks_kernel(const __grid_constant__ PeriodicParams P, cetra_peak *__restrict__ peaks) {
@@ -306,16 +545,18 @@ int build_periodic_plan(int32_t n_lc, int32_t n_dur, cetra_t0_grid grid, const d
     P.t0_start = grid.t0_start; P.t0_stride = grid.t0_stride;
     P.stats_pitch = cetra_stats_pitch(grid.n_t0);
     const size_t row_bytes = static_cast<size_t>(P.stats_pitch) * sizeof(float2);
-    pl->row_in_smem = row_bytes + 16 <= static_cast<size_t>(smem_limit);
-    pl->smem_bytes = pl->row_in_smem ? row_bytes + 16 : 16;
-    // work units: kWarps consecutive periods of one row (one period per warp); see fold_argmax_kernel
+    constexpr size_t kGrpHeader = kGrpHeaderBytes;
+    pl->row_in_smem = row_bytes + kGrpHeader <= static_cast<size_t>(smem_limit);
+    pl->smem_bytes = pl->row_in_smem ? row_bytes + kGrpHeader : 16;
+    // work units: consecutive periods of one row, one period (per-period kernel) or kGrpT periods (grouped
+    // kernel) per warp; see the kernels
     const long long rows = static_cast<long long>(n_lc) * n_dur;
-    constexpr int kWarps = kFoldThreads / 32;
-    P.units_per_row = (n_per + kWarps - 1) / kWarps;
+    const int unit_periods = pl->row_in_smem ? (kGrpThreads / 32) * kGrpT : kFoldThreads / 32;
+    P.units_per_row = (n_per + unit_periods - 1) / unit_periods;
     P.n_units = rows * P.units_per_row;
     if (P.n_units > 0x7fffffffLL - (1LL << 24)) return CETRA_ERR_UNSUPPORTED;   // 32-bit queue head + overshoot
     P.max_claim = std::max(1, 4 * P.units_per_row);
-    const int per_sm = (pl->smem_bytes * 2 + 2048 <= static_cast<size_t>(smem_limit)) ? 2 : 1;
+    const int per_sm = pl->row_in_smem ? 1 : 2;
     pl->grid = static_cast<int>(std::min<long long>(P.n_units, static_cast<long long>(n_sm) * per_sm));
     return CETRA_OK;
 }
@@ -355,9 +596,9 @@ int run_periodic(PeriodicPlan &pl, const float2 *stats_dev, const double *period
     CETRA_CUDA_TRY(cudaMemsetAsync(keys, 0, sizeof(unsigned long long) * (n_keys + 32), st));
     profile_mark(kProfFold, true, st);
     if (pl.row_in_smem) {
-        auto k = fold_argmax_kernel<true>;
+        auto k = fold_group_argmax_kernel;
         CETRA_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes));
-        k<<<pl.grid, kFoldThreads, pl.smem_bytes, st>>>(P);
+        k<<<pl.grid, kGrpThreads, pl.smem_bytes, st>>>(P);
     } else {
         fold_argmax_kernel<false><<<pl.grid, kFoldThreads, pl.smem_bytes, st>>>(P);
     }

@@ -8,6 +8,15 @@ namespace cetra {
 constexpr int kFoldR = 4;            // phase groups (of 32 phases) per warp pass; needs kStatsPad >= 32*kFoldR
 constexpr int kFoldThreads = 1024;
 
+// Grouped fold (rows resident in shared memory): one warp folds kGrpT neighbouring trial periods together.
+constexpr int kGrpT = 2;             // periods per warp
+constexpr int kGrpG = 13;            // consecutive phases per lane; odd => conflict-free 8-byte LDS at a stride of G cells
+constexpr int kGrpS = 7;             // largest spread of a group's epoch offsets served from one register window
+constexpr int kGrpThreads = 512;     // 16 warps x 128 registers
+constexpr size_t kGrpHeaderBytes = 16 + (kGrpThreads / 32) * 32 * 8;   // barrier, claim slot, epoch words
+static_assert(kStatsPad >= 32 * kGrpG + kGrpS + 1, "a pass may read 32*G+S cells past the last t0 cell");
+static_assert(kStatsPad >= 32 * kFoldR, "a pass may read 32*R cells past the last t0 cell");
+
 struct PeriodicParams {
     const float2 *stats;             // [n_lc][n_dur][stats_pitch] (S_wmm, S_wmf), zero in null cells / padding
     const double *periods;           // [n_per] device
@@ -17,14 +26,14 @@ struct PeriodicParams {
     long long stats_pitch;
     double t0_start, t0_stride;
     int n_lc, n_dur, n_t0, n_per;
-    int units_per_row, max_claim;    // unit = kFoldThreads/32 consecutive periods of one row
+    int units_per_row, max_claim;    // unit = periods_per_unit consecutive periods of one row
     long long n_units;
     double durations[CETRA_MAX_DURATIONS];
 };
 
 struct PeriodicPlan {
     PeriodicParams P{};
-    bool row_in_smem = false;
+    bool row_in_smem = false;        // grouped kernel (row in shared memory) or per-period kernel (row in L2)
     size_t smem_bytes = 0;
     int grid = 0;
 };
