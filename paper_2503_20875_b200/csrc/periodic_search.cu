@@ -267,24 +267,43 @@ __device__ __forceinline__ float2 lds_cell(uint32_t addr) {
     return v;
 }
 
+__device__ __forceinline__ int2 lds_int2(uint32_t addr) {
+    int2 v;
+    asm volatile("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
+    return v;
+}
+
+__device__ __forceinline__ void sts_int2(uint32_t addr, int x, int y) {
+    asm volatile("st.shared.v2.s32 [%0], {%1, %2};" ::"r"(addr), "r"(x), "r"(y) : "memory");
+}
+
+// One epoch of a two-period group whose offsets differ by D cells: the G + D cells from the smaller offset on are
+// loaded once; period 0 takes cells [0, G), period 1 cells [D, G + D).
+template <int D, int G>
+__device__ __forceinline__ void fold_epoch(float2 (&acc)[kGrpT][G], uint32_t ptr) {
+    float2 c[G + D];
+#pragma unroll
+    for (int i = 0; i < G + D; ++i) c[i] = lds_cell(ptr + 8u * i);
+#pragma unroll
+    for (int g = 0; g < G; ++g) acc[0][g] = add2(acc[0][g], c[g]);
+#pragma unroll
+    for (int g = 0; g < G; ++g) acc[1][g] = add2(acc[1][g], c[g + D]);
+}
+
 // One pass of a warp over 32*G consecutive phases starting at p0; lane owns phases p0 + lane*G + g.
 // ew: the warp's shared-memory slots for one block of 32 epochs: ew[e] = (off_0, off_1), the offsets of the two
 // periods of the group (off_1 >= off_0 because the periods are sorted).  When off_1 - off_0 <= kGrpS the G + d
 // cells from off_0 on serve both periods from one register window; otherwise each period gathers its own cells.
 template <int G, bool kLastPass>
 __device__ __forceinline__ void fold_group_pass(uint32_t srow, int p0, int n_t0, const GroupPeriods &gp,
-                                                int2 *__restrict__ ew, int lane, float (&best_lr)[kGrpT],
+                                                uint32_t ew, int lane, float (&best_lr)[kGrpT],
                                                 int (&best_p)[kGrpT]) {
-    static_assert(kGrpT == 2, "two periods per warp");
-    constexpr int W = G + kGrpS;
+    static_assert(kGrpT == 2 && kGrpS == 7, "two periods per warp, one switch case per shift");
     float2 acc[kGrpT][G];
-    float2 c[W];
 #pragma unroll
     for (int t = 0; t < kGrpT; ++t)
 #pragma unroll
         for (int g = 0; g < G; ++g) acc[t][g] = make_float2(0.f, 0.f);
-#pragma unroll
-    for (int i = 0; i < W; ++i) c[i] = make_float2(0.f, 0.f);
     const long long limit = static_cast<long long>(n_t0) - 1 - p0;   // off_e <= limit  <=>  p0 + off_e <= I-1
     const uint32_t base = srow + 8u * static_cast<uint32_t>(p0 + lane * G);
     for (int eb = 0;; eb += 32) {
@@ -295,28 +314,32 @@ __device__ __forceinline__ void fold_group_pass(uint32_t srow, int p0, int n_t0,
         const bool ok = o0 <= limit;                                  // r ascending: o0 is the smaller
         const long long cap = 0x0fffffffLL;
         __syncwarp();                                                 // the previous block's words are consumed
-        ew[lane] = make_int2(static_cast<int>(o0 < cap ? o0 : cap), static_cast<int>(o1 < cap ? o1 : cap));
+        sts_int2(ew + 8u * lane, static_cast<int>(o0 < cap ? o0 : cap), static_cast<int>(o1 < cap ? o1 : cap));
         __syncwarp();
         const int cnt = __popc(__ballot_sync(0xffffffffu, ok));       // offsets are monotone in e: a prefix is valid
         for (int t = 0; t < cnt; ++t) {
-            const int2 w = ew[t];                                     // broadcast load
+            const int2 w = lds_int2(ew + 8u * t);                     // broadcast load
             const uint32_t ptr = base + 8u * static_cast<uint32_t>(w.x);
             const int d = w.y - w.x;
-            if (d <= kGrpS) {
+            // one case per shift: load the G + d cells that serve both periods, add them at shift 0 and d
+            switch (d) {
+                case 0: fold_epoch<0, G>(acc, ptr); break;
+                case 1: fold_epoch<1, G>(acc, ptr); break;
+                case 2: fold_epoch<2, G>(acc, ptr); break;
+                case 3: fold_epoch<3, G>(acc, ptr); break;
+                case 4: fold_epoch<4, G>(acc, ptr); break;
+                case 5: fold_epoch<5, G>(acc, ptr); break;
+                case 6: fold_epoch<6, G>(acc, ptr); break;
+                case 7: fold_epoch<7, G>(acc, ptr); break;
+                default: {
+                    // offsets too far apart for one window: each period gathers its own cells
 #pragma unroll
-                for (int i = 0; i < G; ++i) c[i] = lds_cell(ptr + 8u * i);
+                    for (int g = 0; g < G; ++g) acc[0][g] = add2(acc[0][g], lds_cell(ptr + 8u * g));
+                    if (w.y <= limit) {
+                        const uint32_t pu = base + 8u * static_cast<uint32_t>(w.y);
 #pragma unroll
-                for (int i = G; i < W; ++i)
-                    if (i < G + d) c[i] = lds_cell(ptr + 8u * i);
-                add_window<0, G, W>(acc[0], c);
-                add_shifted<G, W>(acc[1], c, d);
-            } else {
-#pragma unroll
-                for (int g = 0; g < G; ++g) acc[0][g] = add2(acc[0][g], lds_cell(ptr + 8u * g));
-                if (w.y <= limit) {
-                    const uint32_t pu = base + 8u * static_cast<uint32_t>(w.y);
-#pragma unroll
-                    for (int g = 0; g < G; ++g) acc[1][g] = add2(acc[1][g], lds_cell(pu + 8u * g));
+                        for (int g = 0; g < G; ++g) acc[1][g] = add2(acc[1][g], lds_cell(pu + 8u * g));
+                    }
                 }
             }
         }
@@ -347,7 +370,7 @@ __global__ void __launch_bounds__(kGrpThreads, 1) fold_group_argmax_kernel(const
     float2 *srow = reinterpret_cast<float2 *>(smem_raw + kGrpHeaderBytes);
     const uint32_t srow_addr = smem_u32(srow);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    int2 *ew = s_ew + warp * 32;
+    const uint32_t ew = smem_u32(s_ew + warp * 32);
 
     if (tid == 0) {
         mbar_init(bar, 1);
