@@ -10,9 +10,9 @@ constexpr int kFoldThreads = 1024;
 
 // Grouped fold (rows resident in shared memory): one warp folds kGrpT neighbouring trial periods together.
 constexpr int kGrpT = 2;             // periods per warp
-constexpr int kGrpG = 13;            // consecutive phases per lane; odd => conflict-free 8-byte LDS at a stride of G cells
+constexpr int kGrpG = 11;            // consecutive phases per lane; odd => conflict-free 8-byte LDS at a stride of G cells
 constexpr int kGrpS = 7;             // largest spread of a group's epoch offsets served from one register window
-constexpr int kGrpThreads = 512;     // 16 warps x 128 registers
+constexpr int kGrpThreads = 640;     // 20 warps x 94 registers (measured best of 448-768 threads, G = 7-15)
 constexpr size_t kGrpHeaderBytes = 16 + (kGrpThreads / 32) * 32 * 8;   // barrier, claim slot, epoch words
 static_assert(kStatsPad >= 32 * kGrpG + kGrpS + 1, "a pass may read 32*G+S cells past the last t0 cell");
 static_assert(kStatsPad >= 32 * kFoldR, "a pass may read 32*R cells past the last t0 cell");
