@@ -10,7 +10,7 @@ light curves.  The workload is BASELINE.json configs[1], the TESS-like 2-min sec
 
   value      light curves/s, inputs resident in HBM when the timed region starts (cetra_search_batched)
   e2e        the same metric through cetra_search_batched_host: pinned HOST buffers, H2D + D2H timed
-  roofline   the dominant kernel (fold_argmax_kernel, periodic search): algorithmic bytes / event time
+  roofline   the dominant kernel (fold_group_argmax_kernel, periodic search): algorithmic bytes / event time
   cpu_baseline  the FP64 oracle on the host cores, on a bounded sample of the same workload
 
 N > 1 (torchrun): every rank searches its own B curves (no data-path collective; "weak" scaling), the
@@ -38,9 +38,9 @@ UNIT = "light curves/s"
 L2_FLUSH_BYTES = 512 << 20
 N_SM, FP32_LANES = 148, 128          # B200: SMs, FP32 FMA lanes per SM (B200_PROFILING.md unit counts)
 SMEM_BYTES_PER_CLK = 128             # shared-memory crossbar bytes/clk/SM (B300_MICROARCH.md, LDS/STS)
-# dram__bytes_read.sum + dram__bytes_write.sum of one fold_argmax_kernel launch over a 14-curve chunk of this
-# workload, from the `ncu --set full` capture summarised in profiles/r01c_fold_full.md (69.4 MB + 3.2 MB)
-NCU_FOLD_DRAM_BYTES_PER_LC = 72.6e6 / 14
+# dram__bytes_read.sum + dram__bytes_write.sum of one fold_group_argmax_kernel launch over a 64-curve chunk of this
+# workload, from the `ncu --set full` capture summarised in profiles/r01h_fold_full.md (332.3 MB + 12.5 MB)
+NCU_FOLD_DRAM_BYTES_PER_LC = 344.8e6 / 64
 
 
 # ----------------------------------------------------------------------------------------------- helpers
@@ -308,10 +308,10 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
                  api="cetra_search_batched_host (pinned host flux/flux_err in, pinned host records out)"),
         gpu_launches=int(launches),
         clocks=clocks.summary(),
-        roofline=dict(bound="hbm", kernel="fold_argmax_kernel", achieved=fold_gbs, peak=peaks["hbm_gbs"],
+        roofline=dict(bound="hbm", kernel="fold_group_argmax_kernel", achieved=fold_gbs, peak=peaks["hbm_gbs"],
                       unit="GB/s", frac=fold_gbs / peaks["hbm_gbs"],
                       traffic=NCU_FOLD_DRAM_BYTES_PER_LC * B * args.steps / fold_launches,
-                      traffic_source="ncu --set full, profiles/r01c_fold_full.md, scaled to the curves per launch",
+                      traffic_source="ncu --set full, profiles/r01h_fold_full.md, scaled to the curves per launch",
                       peak_source=peaks["source"],
                       ms_per_launch=prof["fold_ms"] / fold_launches, launches=int(prof["fold_launches"]),
                       share_of_step=prof["fold_ms"] / ms_dev,
@@ -319,7 +319,10 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
                       served_from="shared memory (one (S_wmm,S_wmf) row per CTA); compulsory HBM traffic is the "
                                   "stats grid once per chunk",
                       smem=dict(achieved=fold_gbs, peak=smem_peak, unit="GB/s", frac=fold_gbs / smem_peak,
-                                peak_derivation="148 SM x 128 B/clk x sm_max_mhz")),
+                                peak_derivation="148 SM x 128 B/clk x sm_max_mhz",
+                                note="algorithmic bytes (8 B per cell) against the crossbar peak; above 1 because a "
+                                     "warp folds two neighbouring periods from one register window, so a loaded "
+                                     "cell serves up to two cells of work (ncu: 82.7 % of the crossbar busy)")),
         roofline_linear=dict(bound="alu", kernel="linear_search_kernel", achieved=lin_tflops, peak=fp32_peak,
                              unit="TFLOP/s", frac=lin_tflops / fp32_peak,
                              peak_derivation="148 SM x 128 FP32 lanes x 2 flop x sm_max_mhz",
