@@ -5,11 +5,12 @@
 //   P3 combine              Z = SB/SA, var = 1/SA, LR = 1/2 SB^2/SA  (= Eq. 4 summed at Z)
 //   P4 argmax               per period: max LR over (duration, phase), ties -> smallest j, then p
 //
-// The combined (depth, var, LR) arrays of a period are never materialised: a warp folds one
-// (period, duration) pair in registers and publishes one packed 64-bit key with atomicMax.
+// The combined (depth, var, LR) arrays of a period are never materialised: a warp folds (period, duration)
+// pairs in registers and publishes one packed 64-bit key per period with atomicMax.
 // A block keeps the (S_wmm, S_wmf) row of one duration in shared memory (one TMA bulk copy per row)
-// and pulls (row, period-segment) work items from a global queue; rows that do not fit in shared
-// memory are gathered from L2 with coalesced read-only loads.
+// and pulls (row, period-segment) work items from a global queue; there a warp folds two neighbouring
+// periods from one register window (fold_group_argmax_kernel).  Rows that do not fit in shared memory
+// are gathered from L2 with coalesced read-only loads, one period per warp (fold_argmax_kernel<false>).
 #include "periodic_search.cuh"
 
 #include <math.h>
@@ -226,36 +227,15 @@ __global__ void __launch_bounds__(kFoldThreads, 1) fold_argmax_kernel(const __gr
 }
 
 // ------------------------------------------------------------------------------- grouped fold (P1-P4)
-// Neighbouring trial periods fold almost the same cells: at epoch e the offsets llrint(e r_k) of kGrpT
-// consecutive periods differ by a few cells.  A warp therefore folds kGrpT periods together; a lane owns
-// G consecutive phases and, per epoch, loads the G + d_max cells that cover all kGrpT periods into a
-// register window once (8-byte LDS at a lane stride of G cells: G odd => conflict-free) and adds them into
-// the kGrpT x G accumulators at the period's shift d_t = off_t(e) - off_0(e), a warp-uniform switch.  One
-// load then feeds up to kGrpT adds, which lifts the kernel off the shared-memory crossbar (the per-period
-// kernel's limit, profiles/r01c).  The per-cell arithmetic, the order of the epoch sum and the offsets
-// (FP64, R11) are exactly those of the per-period kernel.  Epochs whose offsets spread over more than
-// kGrpS cells (long periods) are gathered period by period in the same loop.
-template <int D, int G, int W>
-__device__ __forceinline__ void add_window(float2 (&acc)[G], const float2 (&c)[W]) {
-#pragma unroll
-    for (int g = 0; g < G; ++g) acc[g] = add2(acc[g], c[g + D]);
-}
-
-template <int G, int W>
-__device__ __forceinline__ void add_shifted(float2 (&acc)[G], const float2 (&c)[W], int d) {
-    static_assert(W == G + kGrpS && kGrpS == 7, "one case per shift");
-    switch (d) {
-        case 0: add_window<0, G, W>(acc, c); break;
-        case 1: add_window<1, G, W>(acc, c); break;
-        case 2: add_window<2, G, W>(acc, c); break;
-        case 3: add_window<3, G, W>(acc, c); break;
-        case 4: add_window<4, G, W>(acc, c); break;
-        case 5: add_window<5, G, W>(acc, c); break;
-        case 6: add_window<6, G, W>(acc, c); break;
-        default: add_window<7, G, W>(acc, c); break;
-    }
-}
-
+// Neighbouring trial periods fold almost the same cells: at epoch e the offsets llrint(e r_k) of two consecutive
+// periods differ by a few cells.  A warp therefore folds kGrpT = 2 periods together; a lane owns G consecutive
+// phases and, per epoch, loads the G + d cells that cover both periods once (8-byte LDS at a lane stride of G
+// cells: G odd => conflict-free) and adds them into the two sets of G accumulators at shift 0 and
+// d = off_1(e) - off_0(e), a warp-uniform switch with one straight-line case per shift.  One load then feeds up to
+// two adds, which lifts the kernel off the one-load-per-cell bound of the shared-memory crossbar (the per-period
+// kernel's limit, profiles/r01c).  The per-cell arithmetic, the order of the epoch sum and the offsets (FP64, R11)
+// are exactly those of the per-period kernel.  Epochs whose offsets differ by more than kGrpS cells (long
+// periods) are gathered period by period in the same loop.
 struct GroupPeriods {
     double r[kGrpT];          // period in t0 cells, ascending
     int n_phase[kGrpT];       // R10; 0 for a period that is not searched on this row
