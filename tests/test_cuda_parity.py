@@ -221,6 +221,39 @@ def test_periodic_search_duration_ranges_and_empty_periods(torch_cuda, cetra, or
     assert np.all(pk["j_dur"][ok] >= lo[ok]) and np.all(pk["j_dur"][ok] < hi[ok])
 
 
+@pytest.mark.parametrize("order", ["descending", "shuffled", "duplicates", "single", "far_apart"])
+def test_periodic_search_any_period_order(order, torch_cuda, cetra, oracle_mod):
+    """The fold kernel pairs neighbouring entries of the period array: the records must not depend on how the
+    array is ordered, on an odd count (ragged last pair), on repeated periods, or on pairs whose offsets are too
+    far apart to share a window."""
+    p = _problem(2)
+    g32, g64 = _oracle_periodic_inputs(oracle_mod, 2)
+    rng = np.random.default_rng(77)
+    base = p.periods[rng.choice(p.periods.shape[0], 41, replace=False)]
+    if order == "descending":
+        periods = np.sort(base)[::-1].copy()
+    elif order == "shuffled":
+        periods = base
+    elif order == "duplicates":
+        periods = np.repeat(np.sort(base)[:14], 3)[:41]
+    elif order == "single":
+        periods = base[:1]
+    else:
+        periods = np.array([0.5001, 13.5, 0.7, 9.1, 1.0, 12.0, 0.6])        # every pair spreads over > 7 cells
+    peaks = cetra.cetra_periodic_search(*(_dev(torch_cuda, a) for a in g32), p.t0_start, p.t0_stride, p.durations,
+                                        periods)
+    pk = cetra.peaks_to_numpy(peaks)[0]
+    orc = oracle_mod.periodic_search(g64, p.t0_start, p.t0_stride, p.durations, periods)
+
+    def cell(k, j, ph):
+        return oracle_mod.periodic_cell(g64, p.t0_stride, periods[k], j, ph)
+
+    assert_periodic_parity(pk, orc, cell, what=f"period order {order}")
+    if order == "duplicates":
+        for a in range(0, 39, 3):            # equal periods give equal records
+            assert pk[a] == pk[a + 1] == pk[a + 2]
+
+
 # ------------------------------------------------------------------------- whole path, end to end
 def _gpu_pipeline(torch, cetra, p, periods):
     """Linear search -> sufficient statistics -> periodic search, all on the device (the bench's path)."""
