@@ -163,6 +163,19 @@ int cetra_search_batched(const double *times_host, const void *flux_dev, const v
                          cetra_peak *peaks_dev,
                          void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
 
+/* Same search for a sequence of transit templates ("it may be worth running CETRA across a sequence of values" of
+ * the impact parameter): templates_host is [n_templates][n_template] float32, peaks_dev is
+ * [n_templates][n_lc][n_per]; template t's records are exactly those of cetra_search_batched with that template.
+ * The workspace is the one of cetra_search_batched (the templates are searched one after the other on the stream). */
+int cetra_search_batched_templates(const double *times_host, const void *flux_dev, const void *flux_err_dev,
+                                   cetra_dtype dtype, int64_t n, int32_t n_lc, int32_t lc_chunk,
+                                   const double *durations_host, int32_t n_dur, cetra_t0_grid grid,
+                                   const float *templates_host, int32_t n_template, int32_t n_templates,
+                                   const double *periods_host, int32_t n_per,
+                                   const int32_t *dur_lo_host, const int32_t *dur_hi_host,
+                                   cetra_peak *peaks_dev,
+                                   void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
 /* Same, with the light curves and the result in HOST memory (pinned memory recommended): each chunk is
  * copied host->device, searched, and its records copied device->host on `cuda_stream`; the call
  * synchronises the stream before returning.  The workspace must be

@@ -30,7 +30,7 @@ EXPORTED_SYMBOLS = (
     "cetra_status_string", "cetra_device_info", "cetra_stats_pitch", "cetra_kernel_launch_count",
     "cetra_linear_workspace_bytes", "cetra_linear_search",
     "cetra_periodic_workspace_bytes", "cetra_periodic_search", "cetra_periodic_search_stats",
-    "cetra_search_batched_workspace_bytes", "cetra_search_batched",
+    "cetra_search_batched_workspace_bytes", "cetra_search_batched", "cetra_search_batched_templates",
     "cetra_search_batched_host_workspace_bytes", "cetra_search_batched_host",
     "cetra_profile_enable", "cetra_profile_read",
     "cetra_median_cadence", "cetra_resample_grid", "cetra_resample_workspace_bytes", "cetra_resample",
@@ -108,6 +108,9 @@ def load_library() -> ctypes.CDLL:
     lib.cetra_search_batched.restype = ctypes.c_int
     lib.cetra_search_batched.argtypes = [dp, vp, vp, ctypes.c_int, i64, i32, i32, dp, i32, cetra_t0_grid, fp, i32,
                                          dp, i32, ip, ip, vp, vp, sz, vp]
+    lib.cetra_search_batched_templates.restype = ctypes.c_int
+    lib.cetra_search_batched_templates.argtypes = [dp, vp, vp, ctypes.c_int, i64, i32, i32, dp, i32, cetra_t0_grid, fp,
+                                                   i32, i32, dp, i32, ip, ip, vp, vp, sz, vp]
     lib.cetra_search_batched_host_workspace_bytes.restype = sz
     lib.cetra_search_batched_host_workspace_bytes.argtypes = [dp, i64, i32, i32, ctypes.c_int, dp, i32,
                                                               cetra_t0_grid, i32, i32]
@@ -399,6 +402,37 @@ def cetra_search_batched(times, flux, flux_err, durations, t0_start: float, t0_s
                                       _dp(periods), n_per, lo, hi, peaks.data_ptr(), ws.data_ptr(), ws.numel(),
                                       _stream_ptr(torch, stream))
     _check(rc, "cetra_search_batched")
+    return peaks
+
+
+def cetra_search_batched_templates(times, flux, flux_err, durations, t0_start: float, t0_stride: float, n_t0: int,
+                                   templates, periods, dur_lo=None, dur_hi=None, lc_chunk: int = 0, workspace=None,
+                                   stream=None):
+    """The batched search for every row of `templates` [T][M]; returns peaks [T][B][K][8] int32."""
+    torch = _torch()
+    lib = load_library()
+    flux, flux_err, n_lc, n = _dev_input(torch, flux, flux_err)
+    times, durations, periods = _f64(times), _f64(durations), _f64(periods)
+    tpl = np.ascontiguousarray(templates, dtype=np.float32)
+    if tpl.ndim != 2:
+        raise TypeError("templates must be [T][M]")
+    if times.shape[0] != n:
+        raise CetraError(CETRA_ERR_INVALID_ARG, "cetra_search_batched_templates: len(times) != flux.shape[-1]")
+    lo_arr, lo = _opt_i32(dur_lo)
+    hi_arr, hi = _opt_i32(dur_hi)
+    grid = _grid(t0_start, t0_stride, n_t0)
+    n_dur, n_per = durations.shape[0], periods.shape[0]
+    nbytes = int(lib.cetra_search_batched_workspace_bytes(_dp(times), n, n_lc, int(lc_chunk), _dp(durations), n_dur,
+                                                          grid, tpl.shape[1], n_per))
+    ws = _workspace(torch, nbytes, flux.device, workspace)
+    peaks = torch.empty((tpl.shape[0], n_lc, n_per, 8), dtype=torch.int32, device=flux.device)
+    with torch.cuda.device(flux.device):
+        rc = lib.cetra_search_batched_templates(_dp(times), flux.data_ptr(), flux_err.data_ptr(),
+                                                _dtype_code(torch, flux), n, n_lc, int(lc_chunk), _dp(durations),
+                                                n_dur, grid, tpl.ctypes.data, tpl.shape[1], tpl.shape[0],
+                                                _dp(periods), n_per, lo, hi, peaks.data_ptr(), ws.data_ptr(),
+                                                ws.numel(), _stream_ptr(torch, stream))
+    _check(rc, "cetra_search_batched_templates")
     return peaks
 
 

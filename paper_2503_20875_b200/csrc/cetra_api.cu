@@ -342,6 +342,27 @@ int cetra_search_batched(const double *times_host, const void *flux_dev, const v
     return CETRA_OK;
 }
 
+int cetra_search_batched_templates(const double *times_host, const void *flux_dev, const void *flux_err_dev,
+                                   cetra_dtype dtype, int64_t n, int32_t n_lc, int32_t lc_chunk,
+                                   const double *durations_host, int32_t n_dur, cetra_t0_grid grid,
+                                   const float *templates_host, int32_t n_template, int32_t n_templates,
+                                   const double *periods_host, int32_t n_per, const int32_t *dur_lo_host,
+                                   const int32_t *dur_hi_host, cetra_peak *peaks_dev, void *workspace_dev,
+                                   size_t workspace_bytes, void *cuda_stream) {
+    if (!templates_host || !peaks_dev || n_templates < 1 || n_template < 2 || n_lc < 1 || n_per < 1)
+        return CETRA_ERR_INVALID_ARG;
+    for (int32_t t = 0; t < n_templates; ++t) {               // one search per template
+        const int rc = cetra_search_batched(times_host, flux_dev, flux_err_dev, dtype, n, n_lc, lc_chunk,
+                                            durations_host, n_dur, grid,
+                                            templates_host + static_cast<size_t>(t) * n_template, n_template,
+                                            periods_host, n_per, dur_lo_host, dur_hi_host,
+                                            peaks_dev + static_cast<size_t>(t) * n_lc * n_per, workspace_dev,
+                                            workspace_bytes, cuda_stream);
+        if (rc != CETRA_OK) return rc;
+    }
+    return CETRA_OK;
+}
+
 size_t cetra_search_batched_host_workspace_bytes(const double *times_host, int64_t n, int32_t n_lc, int32_t lc_chunk,
                                                  cetra_dtype dtype, const double *durations_host, int32_t n_dur,
                                                  cetra_t0_grid grid, int32_t n_template, int32_t n_per) {

@@ -359,6 +359,27 @@ def test_batched_equals_single_and_host_variant(torch_cuda, cetra, oracle_mod):
         assert_periodic_parity(pk[b], orc, cell, what=f"batch lc {b}")
 
 
+def test_template_sequence_equals_one_search_per_template(torch_cuda, cetra, oracle_mod):
+    """a sequence of impact parameters.  Every template's records are bit-identical to a search
+    with that template alone, and the grazing template is checked against the oracle."""
+    from cetra_synth import make_survey_batch, tabulate_template
+    p = make_survey_batch(n_lc=3, n_periods=300)
+    flux, err = _dev(torch_cuda, p.flux), _dev(torch_cuda, p.flux_err)
+    tpls = np.stack([tabulate_template(1024, b=b) for b in (0.32, 0.93, 0.99)])      # the paper's three models
+    assert not np.allclose(tpls[0], tpls[2])
+    args = (p.durations, p.t0_start, p.t0_stride, p.n_t0)
+    pk = cetra.cetra_search_batched_templates(p.times, flux, err, *args, tpls, p.periods)
+    assert tuple(pk.shape) == (3, 3, 300, 8)
+    pk = cetra.peaks_to_numpy(pk.reshape(9, 300, 8)).reshape(3, 3, 300)
+    for t in range(3):
+        one = cetra.peaks_to_numpy(cetra.cetra_search_batched(p.times, flux, err, *args, tpls[t], p.periods))
+        assert np.array_equal(one.view(np.uint8), pk[t].view(np.uint8))
+    o = oracle_mod.linear_search(p.times, p.flux[1], p.flux_err[1], *args, tpls[2])
+    orc = oracle_mod.periodic_search(o, p.t0_start, p.t0_stride, p.durations, p.periods)
+    assert_periodic_parity(pk[2][1], orc, lambda k, j, ph: oracle_mod.periodic_cell(o, p.t0_stride, p.periods[k], j, ph),
+                           what="template b = 0.99")
+
+
 def test_bench_configuration_sampled_against_oracle(torch_cuda, cetra, oracle_mod):
     """The launch configuration bench.py times: 64 survey curves of BASELINE configs[1] in one chunk, all 20 000
     periods.  Records of sampled (curve, period) pairs are checked against the oracle one by one, and properties
