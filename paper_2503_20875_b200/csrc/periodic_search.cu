@@ -434,12 +434,16 @@ __global__ void __launch_bounds__(kGrpThreads, 1) fold_group_argmax_kernel(const
                 if (all_on)
                     for (; p0 + 32 * kGrpG <= n_phase_min; p0 += 32 * kGrpG)
                         fold_group_pass<kGrpG, false>(srow_addr, p0, P.n_t0, gp, ew, lane, best_lr, best_p);
-                for (; p0 + 32 * kGrpG < n_phase_max; p0 += 32 * kGrpG)
+                constexpr int kTailG = kGrpG + 2;                      // widest last pass
+                for (; p0 + 32 * kTailG < n_phase_max; p0 += 32 * kGrpG)
                     fold_group_pass<kGrpG, true>(srow_addr, p0, P.n_t0, gp, ew, lane, best_lr, best_p);
-                // the last pass: the narrowest of G = 1, 3, 7, kGrpG phases per lane that covers what is left
+                // the last pass: the narrowest odd number of phases per lane that covers what is left
                 const int left = n_phase_max - p0;
-                if (left > 32 * 7) fold_group_pass<kGrpG, true>(srow_addr, p0, P.n_t0, gp, ew, lane, best_lr, best_p);
-                else if (left > 32 * 3) fold_group_pass<7, true>(srow_addr, p0, P.n_t0, gp, ew, lane, best_lr, best_p);
+                if (left > 32 * 11) fold_group_pass<13, true>(srow_addr, p0, P.n_t0, gp, ew, lane, best_lr, best_p);
+                else if (left > 32 * 9) fold_group_pass<11, true>(srow_addr, p0, P.n_t0, gp, ew, lane, best_lr, best_p);
+                else if (left > 32 * 7) fold_group_pass<9, true>(srow_addr, p0, P.n_t0, gp, ew, lane, best_lr, best_p);
+                else if (left > 32 * 5) fold_group_pass<7, true>(srow_addr, p0, P.n_t0, gp, ew, lane, best_lr, best_p);
+                else if (left > 32 * 3) fold_group_pass<5, true>(srow_addr, p0, P.n_t0, gp, ew, lane, best_lr, best_p);
                 else if (left > 32) fold_group_pass<3, true>(srow_addr, p0, P.n_t0, gp, ew, lane, best_lr, best_p);
                 else if (left > 0) fold_group_pass<1, true>(srow_addr, p0, P.n_t0, gp, ew, lane, best_lr, best_p);
                 // P4 across the warp: larger lr wins, ties -> smaller phase; one atomicMax per period

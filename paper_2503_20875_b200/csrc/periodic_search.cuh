@@ -14,7 +14,7 @@ constexpr int kGrpG = 11;            // consecutive phases per lane; odd => conf
 constexpr int kGrpS = 7;             // largest spread of a group's epoch offsets served from one register window
 constexpr int kGrpThreads = 640;     // 20 warps x 94 registers (measured best of 448-768 threads, G = 7-15)
 constexpr size_t kGrpHeaderBytes = 16 + (kGrpThreads / 32) * 32 * 8;   // barrier, claim slot, epoch words
-static_assert(kStatsPad >= 32 * kGrpG + kGrpS + 1, "a pass may read 32*G+S cells past the last t0 cell");
+static_assert(kStatsPad >= 32 * (kGrpG + 2) + kGrpS + 1, "the widest (last) pass may read 32*(G+2)+S cells past the last t0 cell");
 static_assert(kStatsPad >= 32 * kFoldR, "a pass may read 32*R cells past the last t0 cell");
 
 struct PeriodicParams {
