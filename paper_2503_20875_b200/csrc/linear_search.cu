@@ -156,6 +156,14 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
         issue(0, true);
     }
     __syncthreads();
+    if (P.stats && tile == P.tiles_per_row - 1) {               // zero the row padding (while the fill is in flight)
+        const long long prow = lc * P.n_dur + j;
+        for (long long i = P.n_t0 + tid; i < P.stats_pitch; i += WARPS * 32)
+            P.stats[prow * P.stats_pitch + i] = make_float2(0.f, 0.f);
+    }
+    // a warp whose 32*R cells all lie past the last t0 cell has nothing to compute (last tile of a row); with
+    // several polyphase branches every warp stays for the block-wide barriers between the branches
+    if (q == 1 && i_blk + static_cast<long long>(warp) * (32 * R) >= P.n_t0) return;
 
     // Two-level summation: the running FFMA accumulators are folded into a second set every kFlush tap
     // groups (and at the end of every polyphase branch), so that no FP32 sum runs over more than
@@ -228,10 +236,6 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
             if (P.dlogL) P.dlogL[row * P.n_t0 + i] = null_cell ? nanv : 0.5f * bsum * depth;
             if (P.stats) P.stats[row * P.stats_pitch + i] = null_cell ? make_float2(0.f, 0.f) : ab;
         }
-    }
-    if (P.stats && tile == P.tiles_per_row - 1) {               // zero the row padding
-        for (long long i = P.n_t0 + tid; i < P.stats_pitch; i += WARPS * 32)
-            P.stats[row * P.stats_pitch + i] = make_float2(0.f, 0.f);
     }
 }
 
