@@ -10,7 +10,8 @@
 // A block keeps the (S_wmm, S_wmf) row of one duration in shared memory (one TMA bulk copy per row)
 // and pulls (row, period-segment) work items from a global queue; there a warp folds two neighbouring
 // periods from one register window (fold_group_argmax_kernel).  Rows that do not fit in shared memory
-// are gathered from L2 with coalesced read-only loads, one period per warp (fold_argmax_kernel<false>).
+// are gathered from global memory with coalesced read-only loads, one period per warp (fold_argmax_kernel<false>;
+// neighbouring warps fold neighbouring periods, so 96 % of the sectors hit in L1).
 #include "periodic_search.cuh"
 
 #include <math.h>
@@ -132,15 +133,12 @@ __device__ __forceinline__ void fold_period(const float2 *__restrict__ row, int 
     int p0 = 0;
     for (; p0 + 32 * kFoldR <= n_phase; p0 += 32 * kFoldR)
         fold_pass<kFoldR, kSmemRow>(row, p0, n_t0, n_phase, r, r_floor, b0, lane, best_lr, best_p);
-    static_assert(kFoldR == 4, "the remainder switch below covers 1..kFoldR groups");
-    const int groups = (n_phase - p0 + 31) >> 5;
-    switch (groups) {
-        case 1: fold_pass<1, kSmemRow>(row, p0, n_t0, n_phase, r, r_floor, b0, lane, best_lr, best_p); break;
-        case 2: fold_pass<2, kSmemRow>(row, p0, n_t0, n_phase, r, r_floor, b0, lane, best_lr, best_p); break;
-        case 3: fold_pass<3, kSmemRow>(row, p0, n_t0, n_phase, r, r_floor, b0, lane, best_lr, best_p); break;
-        case 4: fold_pass<4, kSmemRow>(row, p0, n_t0, n_phase, r, r_floor, b0, lane, best_lr, best_p); break;   // 97..127 phases left
-        default: break;
-    }
+    static_assert(kFoldR == 8, "the remainder below covers 1..kFoldR groups by powers of two");
+    const int groups = (n_phase - p0 + 31) >> 5;                  // the last pass: the next power of two of groups
+    if (groups > 4) fold_pass<8, kSmemRow>(row, p0, n_t0, n_phase, r, r_floor, b0, lane, best_lr, best_p);
+    else if (groups > 2) fold_pass<4, kSmemRow>(row, p0, n_t0, n_phase, r, r_floor, b0, lane, best_lr, best_p);
+    else if (groups > 1) fold_pass<2, kSmemRow>(row, p0, n_t0, n_phase, r, r_floor, b0, lane, best_lr, best_p);
+    else if (groups > 0) fold_pass<1, kSmemRow>(row, p0, n_t0, n_phase, r, r_floor, b0, lane, best_lr, best_p);
     // warp argmax: larger lr wins, ties -> smaller phase
 #pragma unroll
     for (int s = 16; s > 0; s >>= 1) {
@@ -563,7 +561,7 @@ int build_periodic_plan(int32_t n_lc, int32_t n_dur, cetra_t0_grid grid, const d
     P.n_units = rows * P.units_per_row;
     if (P.n_units > 0x7fffffffLL - (1LL << 24)) return CETRA_ERR_UNSUPPORTED;   // 32-bit queue head + overshoot
     P.max_claim = std::max(1, 4 * P.units_per_row);
-    const int per_sm = pl->row_in_smem ? 1 : 2;
+    const int per_sm = 1;                                     // both fold kernels fill an SM with one CTA
     pl->grid = static_cast<int>(std::min<long long>(P.n_units, static_cast<long long>(n_sm) * per_sm));
     return CETRA_OK;
 }

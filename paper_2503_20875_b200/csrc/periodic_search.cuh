@@ -5,8 +5,8 @@
 
 namespace cetra {
 
-constexpr int kFoldR = 4;            // phase groups (of 32 phases) per warp pass; needs kStatsPad >= 32*kFoldR
-constexpr int kFoldThreads = 1024;
+constexpr int kFoldR = 8;            // phase groups (of 32 phases) per warp pass; needs kStatsPad >= 32*kFoldR
+constexpr int kFoldThreads = 512;    // 16 warps x 128 registers: 8 x 4 loads in flight per lane (the kernel is latency-bound)
 
 // Grouped fold (rows resident in shared memory): one warp folds kGrpT neighbouring trial periods together.
 constexpr int kGrpT = 2;             // periods per warp
