@@ -449,10 +449,18 @@ def run_configs(args):
             og_ms = med_ms(lambda: cetra.cetra_linear_search(p.times, flux, err, p.durations, p.times[0], stride, n_t0,
                                                              p.template, want_grids=False, want_stats=True), reps)
             evals = wc["template_evals"] * (n_t0 / p.n_t0)
+            og = cetra.cetra_linear_search(p.times, flux, err, p.durations, p.times[0], stride, n_t0, p.template,
+                                           want_grids=False, want_stats=True)
+            ogp_ms = med_ms(lambda: cetra.cetra_periodic_search_stats(og.stats, n_t0, p.times[0], stride, p.durations,
+                                                                      p.periods), max(1, min(reps, 3)))
+            og_bytes = 8.0 * wc["pairs"] * n_t0
             print(json.dumps(dict(workload="configs[1] on the paper's default t0 grid (stride = 1 % of the shortest "
-                                           "duration, off the sample grid): linear_general_kernel",
+                                           "duration, off the sample grid): linear_general_kernel, then the "
+                                           "large-row fold kernel (1.05 MB rows)",
                                   n_t0=n_t0, linear_ms=og_ms, template_evals_per_s=evals / (og_ms * 1e-3),
-                                  bound="fp64 (one IEEE division per template evaluation)")), flush=True)
+                                  bound="fp64 index arithmetic (one IEEE division per template evaluation)",
+                                  periodic_ms=ogp_ms, fold_algorithmic_gbs=og_bytes / (ogp_ms * 1e-3) / 1e9,
+                                  light_curves_per_s=1e3 / (og_ms + ogp_ms))), flush=True)
     # setup kernels: resampling 64 irregular light curves of 200 000 observations (HBM-bound streaming)
     t, f, e = make_irregular_batch(n_lc=64, n=200000)
     td, fd, ed = (torch.from_numpy(a).to(dev) for a in (t, f, e))
