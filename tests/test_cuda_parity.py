@@ -469,6 +469,32 @@ def test_whole_path_off_grid_t0(torch_cuda, cetra, oracle_mod):
                          o.depth, o.depth_var, o.dlogL, what="config 1 off-grid grids")
 
 
+def test_large_row_fold_all_remainder_widths(torch_cuda, cetra, oracle_mod):
+    """Rows larger than shared memory (t0 stride = half a cadence on config-2 data: 39 455 cells, 316 KB per row)
+    take the per-period fold kernel; periods are chosen so that the number of phases modulo the 256-phase pass
+    leaves every remainder width (1, 2, 3-4, 5-8 groups of 32) and the exact multiples."""
+    import oracle as oracle_pkg
+    p = _problem(2)
+    stride = 0.5 * p.cadence
+    n_t0 = 2 * p.n - 1
+    durations = p.durations[[0, 7, 15, 22, 29]]
+    flux, err = _dev(torch_cuda, p.flux), _dev(torch_cuda, p.flux_err)
+    lin = cetra.cetra_linear_search(p.times, flux, err, durations, p.t0_start, stride, n_t0, p.template)
+    assert cetra.cetra_stats_pitch(n_t0) * 8 > 232448          # the row cannot be staged in shared memory
+    # numbers of phases: 256 m + {0, 1, 20, 33, 64, 65, 100, 128, 129, 200, 255} for a few m
+    n_phase = np.array([256 * m + r for m in (3, 4, 9) for r in (0, 1, 20, 33, 64, 65, 100, 128, 129, 200, 255)])
+    periods = (n_phase - 0.37) * stride
+    assert np.array_equal(np.ceil(periods / stride).astype(int), n_phase)
+    periods = np.concatenate([periods, [13.7, 6.01, 27.0, 40.0]])     # few epochs, a single epoch, longer than the data
+    peaks = cetra.cetra_periodic_search(lin.depth, lin.depth_var, lin.dlogL, p.t0_start, stride, durations, periods)
+    pk = cetra.peaks_to_numpy(peaks)[0]
+    g32 = oracle_pkg.LinearGrids(*(a.cpu().numpy().astype(np.float64) for a in (lin.depth, lin.depth_var, lin.dlogL)))
+    orc = oracle_mod.periodic_search(g32, p.t0_start, stride, durations, periods)
+    res = assert_periodic_parity(pk, orc, lambda k, j, ph: oracle_mod.periodic_cell(g32, stride, periods[k], j, ph),
+                                 what="large-row fold")
+    print("large-row fold", res)
+
+
 # ------------------------------------------------------------------------------- error behaviour
 def test_status_codes_on_device(torch_cuda, cetra):
     p = _problem(1)
