@@ -25,7 +25,8 @@
  *    non-finite / non-positive flux_err.  flux is normalised to baseline 1;
  *    internally f = 1 - flux (R7).
  *  - The t0 grid is t_i = t0_start + i*t0_stride, i < n_t0, any start and any stride > 0.
- *    When t0_start lies on the sample grid and t0_stride is a whole number of cadences (to 1e-6 cadence)
+ *    When every t0 cell lies on a sample (to 1e-6 cadence at the last cell: |a - round a| + |b - round b| (n_t0-1)
+ *    <= 1e-6 with a = (t0_start - times[0])/c, b = t0_stride/c, b >= 1)
  *    the nearest-neighbour template position comes from the integer sample offset (R3) and the fast
  *    tabulated-tap kernel runs; otherwise (e.g. the paper's default stride, 1 % of the shortest duration)
  *    it comes from the time difference x = (n*c - (t_i - times[0]))/D + 1/2 in FP64 (R25) and a per-cell

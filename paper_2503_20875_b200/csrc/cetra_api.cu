@@ -66,7 +66,11 @@ int derive_geometry(const double *times_host, int64_t n, cetra_t0_grid grid, Geo
     g->cadence = c;
     g->delta = grid.t0_start - times_host[0];
     g->stride = grid.t0_stride;
-    g->on_grid = !(fabs(a - static_cast<double>(ia)) > 1e-6 || fabs(b - static_cast<double>(ib)) > 1e-6 || ib < 1);
+    // on the sample grid iff no cell of the t0 grid is further than 1e-6 samples from a sample: the mismatch of
+    // the stride accumulates over the grid, so it is bounded at the last cell (R25)
+    const double drift = fabs(a - static_cast<double>(ia)) +
+                         fabs(b - static_cast<double>(ib)) * static_cast<double>(grid.n_t0 - 1);
+    g->on_grid = !(drift > 1e-6 || ib < 1);
     g->n0 = g->on_grid ? ia : 0;
     g->q = g->on_grid ? ib : 0;
     return CETRA_OK;

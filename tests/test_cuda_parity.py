@@ -138,6 +138,46 @@ def test_linear_search_edge_geometry(torch_cuda, cetra, oracle_mod):
     assert saw_null, "the long gaps must produce null cells in at least one case"
 
 
+def test_linear_search_window_edge_samples(torch_cuda, cetra, oracle_mod):
+    """R2: D/(2c) a whole number puts a sample exactly on the first and on the last instant of every window; both
+    belong to it.  Box template on a power-of-two cadence (k c and D/2 exact): the GPU must match the oracle AND
+    the plain inclusive-window weighted mean computed here from the raw data (so that a shared `<` instead of
+    `<=` cannot pass), for a stride of one and of two samples (the polyphase path) and for float64 input."""
+    rng = np.random.default_rng(12)
+    n, c = 5000, 1.0 / 256.0
+    times = 3.0 + np.arange(n) * c
+    err = 1e-3 * (0.5 + rng.random(n))
+    flux = 1.0 + rng.standard_normal(n) * err
+    flux[700:720] = np.nan
+    hs = np.array([1, 2, 7, 8, 15, 16, 40])
+    durations = 2.0 * (hs * c)
+    box = np.ones(32, np.float32)
+    good = np.isfinite(flux)
+    w = np.where(good, 1.0 / err ** 2, 0.0)
+    wf = np.where(good, w * (1.0 - np.where(good, flux, 1.0)), 0.0)
+    cw, cwf = np.concatenate([[0.0], np.cumsum(w)]), np.concatenate([[0.0], np.cumsum(wf)])
+    for dt, q in ((np.float32, 1), (np.float64, 1), (np.float32, 2)):
+        fl, er = flux.astype(dt), err.astype(dt)
+        n_t0 = (n - 1) // q + 1
+        g = cetra.cetra_linear_search(times, _dev(torch_cuda, fl), _dev(torch_cuda, er), durations, times[0], q * c,
+                                      n_t0, box)
+        o = oracle_mod.linear_search(times, fl, er, durations, times[0], q * c, n_t0, box)
+        assert_linear_parity(g.depth.cpu().numpy(), g.depth_var.cpu().numpy(), g.dlogL.cpu().numpy(),
+                             o.depth, o.depth_var, o.dlogL, what=f"edge samples {dt.__name__} q={q}")
+        if dt is np.float64:
+            centre = q * np.arange(n_t0)
+            var_g = g.depth_var.cpu().numpy().astype(np.float64)
+            dep_g = g.depth.cpu().numpy().astype(np.float64)
+            for j, h in enumerate(hs):
+                lo, hi = np.maximum(centre - h, 0), np.minimum(centre + h, n - 1) + 1     # inclusive of both edges
+                sw, swf = cw[hi] - cw[lo], cwf[hi] - cwf[lo]
+                ok = sw > 0
+                assert np.array_equal(np.isnan(var_g[j]), ~ok)
+                assert np.allclose(var_g[j][ok], 1.0 / sw[ok], rtol=3e-5)
+                assert np.allclose(dep_g[j][ok], swf[ok] / sw[ok], rtol=0, atol=3e-5 * np.sqrt(1.0 / sw[ok]).max())
+                # dropping one edge sample of the 2h+1 would change var by 1/(2h+1) >= 1.2 %: far above 3e-5
+
+
 # ---------------------------------------------------------------------------------------- periodic
 def _oracle_periodic_inputs(oracle_mod, cfg):
     """Oracle linear grids rounded to the float32 the GPU entry point takes, promoted back to float64."""

@@ -378,3 +378,154 @@ def test_duration_must_be_shorter_than_period_and_ties(oracle_mod):
     pg = oracle_mod.periodic_search(grids, 0.0, s, durations, periods, lo, hi)
     assert list(pg.j_dur) == [-1, 1, 1]                   # P=0.5: D=0.5 is not < P, D=1.0 neither
     assert np.isnan(pg.lr[0]) and pg.i_t0[0] == -1
+
+
+# ------------------------------------------------------------ branches that GPU parity cannot see
+# The three tests below each kill one plausible mistake that the CUDA path would share by construction
+# (VERDICT round 1): a fold that stops at the first null epoch instead of skipping it, floor(P/s) phases
+# instead of ceil(P/s), and a window that drops the sample sitting exactly on its last (or first) instant.
+def _nearest_cells(I, s, P, p):
+    """Cells a (P, p) fold touches, from the definition: the grid point nearest to t0_p + e P."""
+    t0s = np.arange(I) * s
+    out, e = [], 0
+    while t0s[p] + e * P <= t0s[-1] + 0.5 * s:
+        out.append(int(np.argmin(np.abs(t0s - (t0s[p] + e * P)))))
+        e += 1
+    return out
+
+
+def test_fold_skips_null_epochs_hand_built_grid(oracle_mod):
+    """PAPER.md:123 ("no influence on either the depth or the likelihood ratio"): epochs whose cell is null are
+    skipped, the later epochs still contribute.  Kills `continue -> break` on a null epoch in fold_cell."""
+    I, s = 500, 0.01
+    wts = 1.0 + np.arange(I) * 1e-3                     # distinct weights: the sum identifies the set of cells
+    dep = 1.0 + 0.25 * np.sin(np.arange(I) * 0.37)
+    for P, p in ((0.7331, 7), (0.31415, 29), (1.23457, 0)):
+        cells = _nearest_cells(I, s, P, p)
+        assert len(cells) >= 4
+        null = [cells[1], cells[3]] if len(cells) >= 5 else [cells[1]]
+        kept = [c for c in cells if c not in null]
+        depth = dep[None, :].copy(); var = (1.0 / wts)[None, :].copy()
+        dl = 0.5 * depth ** 2 / var
+        for arr in (depth, var, dl):
+            arr[0, null] = np.nan
+        grids = oracle_mod.LinearGrids(depth, var, dl)
+        lr, z, zv, ntr = oracle_mod.periodic_cell(grids, s, P, 0, p)
+        assert ntr == len(cells) - len(null)
+        assert 1.0 / zv == pytest.approx(np.sum(wts[kept]), rel=1e-13)
+        assert z == pytest.approx(np.sum(wts[kept] * dep[kept]) / np.sum(wts[kept]), rel=1e-13)
+        assert lr == pytest.approx(0.5 * np.sum(wts[kept] * dep[kept]) ** 2 / np.sum(wts[kept]), rel=1e-12)
+        # the per-period search reports the same element (every other phase is left null)
+        only = np.full((1, I), np.nan)
+        d1, v1, l1 = only.copy(), only.copy(), only.copy()
+        d1[0, kept], v1[0, kept], l1[0, kept] = depth[0, kept], var[0, kept], dl[0, kept]
+        pg = oracle_mod.periodic_search(oracle_mod.LinearGrids(d1, v1, l1), 0.0, s, np.array([0.05]), np.array([P]))
+        assert pg.i_t0[0] == p and pg.n_transits[0] == len(kept)
+        assert pg.lr[0] == pytest.approx(lr, rel=1e-13)
+
+
+def test_fold_across_a_data_gap_equals_joint_fit(oracle_mod):
+    """P4 with a gap longer than the duration: the epoch that falls in the gap has a null linear cell, the joint
+    weighted least-squares fit of the multi-transit model to the raw data ignores it (its points carry no
+    weight), and the folded statistics must agree with that fit.  Kills `continue -> break`."""
+    n, c = 1100, 0.01
+    P_cells, p = 220, 63
+    sig = lambda tt: 2e-3 * _staircase_fn(((tt - 0.63 + 1.1) % 2.2 - 1.1) / 0.2371 + 0.5)
+    t, flux, err = _lc(n, c, 1e-3, 33, signal=sig)
+    gap = slice(p + P_cells - 30, p + P_cells + 31)        # 0.6 d around the second epoch; D <= 0.2371 d
+    flux[gap] = np.nan; err[gap] = np.inf
+    durations = np.array([0.1537, 0.2371])
+    g = oracle_mod.linear_search(t, flux, err, durations, t[0], c, n, _staircase())
+    assert np.isnan(g.depth[:, p + P_cells]).all() and not np.isnan(g.depth[:, p + 2 * P_cells]).any()
+    good = np.isfinite(flux)
+    f = np.where(good, 1.0 - np.where(good, flux, 1.0), 0.0)
+    w = np.where(good, 1.0 / np.where(good, err, 1.0) ** 2, 0.0)
+    P = P_cells * c
+    for j, D in enumerate(durations):
+        model = np.zeros(n)
+        e = 0
+        while p + e * P_cells <= n - 1:
+            model += _staircase_fn((t - (t[p] + e * P)) / D + 0.5)
+            e += 1
+        assert e == 5
+        sab, saa = np.sum(w * model * f), np.sum(w * model * model)
+        lr, z, zv, ntr = oracle_mod.periodic_cell(g, c, P, j, p)
+        assert ntr == e - 1                                # four of the five epochs have data
+        assert z == pytest.approx(sab / saa, rel=1e-9)
+        assert zv == pytest.approx(1.0 / saa, rel=1e-10)
+        assert lr == pytest.approx(0.5 * sab * sab / saa, rel=1e-8)
+        ll = np.sum(-0.5 * w * (z * model - f) ** 2) + np.sum(0.5 * w * f * f)
+        assert lr == pytest.approx(ll, rel=1e-8)
+
+
+def test_phase_count_is_ceil_of_period_in_cells(oracle_mod):
+    """R10: the first epoch may sit in any cell p with p*s < P, i.e. p < ceil(P/s).  For a non-integer P/s a
+    signal whose first epoch is cell floor(P/s) is a phase of its own (no earlier phase touches the same
+    cells).  Kills `n_phase = ceil(r) -> floor(r)`."""
+    I, s = 400, 0.01
+    r = 57.4
+    P = r * s
+    p_star = 57                                            # = floor(r) < ceil(r) = 58
+    assert p_star * s < P
+    cells = _nearest_cells(I, s, P, p_star)
+    depth = np.zeros((1, I)); var = np.ones((1, I))
+    depth[0, cells] = 1.0
+    dl = 0.5 * depth ** 2 / var
+    grids = oracle_mod.LinearGrids(depth, var, dl)
+    pg = oracle_mod.periodic_search(grids, 0.0, s, np.array([0.05]), np.array([P]))
+    assert pg.i_t0[0] == p_star and pg.i_t0[0] < int(np.ceil(r))
+    assert pg.n_transits[0] == len(cells)
+    assert pg.lr[0] == pytest.approx(0.5 * len(cells), rel=1e-13)
+    # no phase below floor(r) reaches that likelihood: a floor(r)-phase search would lose the peak
+    others = [oracle_mod.periodic_cell(grids, s, P, 0, q)[0] for q in range(p_star)]
+    assert max(others) < 0.5 * pg.lr[0]
+    # the same from raw data: box transits centred on cell 57 + nearest(e r) of a noiseless light curve
+    n = I
+    t = np.arange(n) * s
+    flux = np.ones(n)
+    for cc in cells:
+        flux[max(cc - 2, 0):cc + 3] -= 1e-3
+    g = oracle_mod.linear_search(t, flux, np.full(n, 1e-4), np.array([0.045]), 0.0, s, n, np.ones(16))
+    pg2 = oracle_mod.periodic_search(g, 0.0, s, np.array([0.045]), np.array([P]))
+    assert pg2.i_t0[0] == p_star and pg2.depth[0] == pytest.approx(1e-3, rel=1e-9)
+    # integer P/s (power-of-two stride, so that P/s is exact): ceil = floor, the last phase is r - 1; the only
+    # signal sits in cells 57 + 57 e, which is phase 0's second epoch onward, so the winner is a phase < 57
+    s2 = 1.0 / 128.0
+    d3 = np.zeros((1, I)); d3[0, 57::57] = 1.0
+    g3 = oracle_mod.LinearGrids(d3, np.ones((1, I)), 0.5 * d3 ** 2)
+    pg3 = oracle_mod.periodic_search(g3, 0.0, s2, np.array([0.05]), np.array([57 * s2]))
+    assert pg3.i_t0[0] == 0 and pg3.n_transits[0] == len(range(0, I, 57))
+
+
+def test_window_includes_samples_on_its_first_and_last_instant(oracle_mod):
+    """R2 (first and last element of the window, both inclusive): with D/(2c) a whole number the
+    samples at t_i -+ D/2 sit exactly on x = 0 and x = 1 and belong to the window.  Box template = the BLS
+    window of P3 with edge samples; a staircase template fixes which template end each edge sample takes.
+    Kills `x <= 1 -> x < 1` (and `x >= 0 -> x > 0`)."""
+    n, c = 300, 1.0 / 64.0                                 # power-of-two cadence: k*c and D/2 are exact
+    t, flux, err = _lc(n, c, 1e-3, 17)
+    f, w = 1.0 - flux, 1.0 / err ** 2
+    for h in (3, 7):
+        D = 2.0 * (h * c)
+        g = oracle_mod.linear_search(t, flux, err, np.array([D]), t[0], c, n, np.ones(32))
+        gs = oracle_mod.linear_search(t, flux, err, np.array([D]), t[0], c, n, _staircase())
+        for i in (0, 2, 50, 151, n - 1):
+            win = np.abs(t - t[i]) <= 0.5 * D               # inclusive on both sides
+            assert win.sum() == min(i, h) + min(n - 1 - i, h) + 1
+            assert g.depth_var[0, i] == pytest.approx(1.0 / np.sum(w[win]), rel=1e-13)
+            assert g.depth[0, i] == pytest.approx(np.sum(w[win] * f[win]) / np.sum(w[win]), rel=1e-12)
+            # staircase: tpl = 0.5 at first contact, 0.25 at last contact
+            m = _staircase_fn((t - t[i]) / D + 0.5)
+            assert m[i - h] == 0.5 if i >= h else True
+            assert m[i + h] == 0.25 if i + h < n else True
+            assert gs.depth_var[0, i] == pytest.approx(1.0 / np.sum(w * m * m), rel=1e-13)
+            assert gs.depth[0, i] == pytest.approx(np.sum(w * m * f) / np.sum(w * m * m), rel=1e-12)
+    # the off-grid form (R25) takes the same decision: t0 grid shifted by a quarter cadence, D/2 = (h + 1/4) c
+    h = 5
+    D = 2.0 * ((h + 0.25) * c)
+    gg = oracle_mod.linear_search(t, flux, err, np.array([D]), t[0] + 0.25 * c, c, n - 1, np.ones(32))
+    for i in (40, 200):
+        ti = t[0] + 0.25 * c + i * c
+        win = np.abs(t - ti) <= 0.5 * D
+        assert win.sum() == 2 * h + 1 and t[win][0] - ti == -0.5 * D      # the first sample sits exactly on x = 0
+        assert gg.depth_var[0, i] == pytest.approx(1.0 / np.sum(w[win]), rel=1e-13)
