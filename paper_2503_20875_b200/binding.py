@@ -79,8 +79,8 @@ def load_library() -> ctypes.CDLL:
     if _lib is not None:
         return _lib
     path = _build.LIB_PATH
-    if not os.path.exists(path) or os.environ.get("CETRA_REBUILD") == "1":
-        path = _build.build()
+    if not os.path.exists(path) or os.environ.get("CETRA_REBUILD") == "1" or (_build.stale() and _build.have_nvcc()):
+        path = _build.build(force=os.environ.get("CETRA_REBUILD") == "1")
     lib = ctypes.CDLL(path)
     vp, dp, fp, ip = ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.c_void_p, ctypes.c_void_p
     i32, i64, sz = ctypes.c_int32, ctypes.c_int64, ctypes.c_size_t

@@ -29,7 +29,7 @@ def _nvcc() -> str:
     return "nvcc"
 
 
-def _stale() -> bool:
+def stale() -> bool:
     if not os.path.exists(LIB_PATH):
         return True
     built = os.path.getmtime(LIB_PATH)
@@ -37,9 +37,15 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > built for d in deps)
 
 
+def have_nvcc() -> bool:
+    import shutil
+    n = _nvcc()
+    return os.path.exists(n) if os.path.isabs(n) else shutil.which(n) is not None
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     """Build libcetra_b200.so if it is missing or older than its sources; return its path."""
-    if not (force or _stale()):
+    if not (force or stale()):
         return LIB_PATH
     cmd = [_nvcc(), *NVCC_FLAGS, "-I", INCLUDE, "-I", CSRC]
     if verbose:
