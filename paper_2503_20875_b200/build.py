@@ -14,11 +14,11 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_PKG)
 CSRC = os.path.join(_PKG, "csrc")
 INCLUDE = os.path.join(_ROOT, "include")
-LIB_PATH = os.path.join(_PKG, "libcetra_b200.so")
-SOURCES = ["cetra_api.cu", "linear_search.cu", "periodic_search.cu", "setup_steps.cu"]
+LIB_PATH = os.environ.get("CETRA_LIB_PATH") or os.path.join(_PKG, "libcetra_b200.so")
+SOURCES = ["cetra_api.cu", "linear_search.cu", "periodic_search.cu", "fold_pair.cu", "fold_stream.cu", "setup_steps.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-    "-shared", "-Xcompiler", "-fPIC",
+    "-shared", "-Xcompiler", "-fPIC", "--threads", "0",
 ]
 
 
@@ -47,7 +47,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     """Build libcetra_b200.so if it is missing or older than its sources; return its path."""
     if not (force or stale()):
         return LIB_PATH
-    cmd = [_nvcc(), *NVCC_FLAGS, "-I", INCLUDE, "-I", CSRC]
+    cmd = [_nvcc(), *NVCC_FLAGS, "-I", INCLUDE, "-I", CSRC] + os.environ.get("CETRA_NVCC_EXTRA", "").split()
     if verbose:
         cmd += ["-Xptxas", "-v"]
     cmd += [os.path.join(CSRC, s) for s in SOURCES] + ["-o", LIB_PATH]

@@ -5,21 +5,24 @@
 
 namespace cetra {
 
-constexpr int kFoldR = 8;            // phase groups (of 32 phases) per warp pass; needs kStatsPad >= 32*kFoldR
-constexpr int kFoldThreads = 512;    // 16 warps x 128 registers: 8 x 4 loads in flight per lane (the kernel is latency-bound)
-
-// Grouped fold (rows resident in shared memory): one warp folds kGrpT neighbouring trial periods together.
+// Pair fold (rows resident in shared memory): one warp folds kGrpT neighbouring trial periods together.
 constexpr int kGrpT = 2;             // periods per warp
 constexpr int kGrpG = 11;            // consecutive phases per lane; odd => conflict-free 8-byte LDS at a stride of G cells
-constexpr int kGrpS = 7;             // largest spread of a group's epoch offsets served from one register window
-constexpr int kGrpThreads = 640;     // 20 warps x 94 registers (measured best of 448-768 threads, G = 7-15)
-constexpr size_t kGrpHeaderBytes = 16 + (kGrpThreads / 32) * 32 * 8;   // barrier, claim slot, epoch words
+constexpr int kGrpS = 7;             // streamed kernel: largest offset difference of a pair served from one register window
+constexpr int kGrpThreads = 640;     // 20 warps x 96 registers
+constexpr size_t kGrpHeaderBytes = 16 + (kGrpThreads / 32) * 64 * 8;   // barrier, claim slot, epoch words (2 blocks per warp)
+// Streamed fold (rows that do not fit in shared memory): 19 consumer warps + one producer warp, a ring of stages
+// (640 threads keep the 96-register budget the two-period register window needs).
+constexpr int kStrThreads = 640;
+constexpr int kStrUnitPeriods = (kStrThreads / 32 - 1) * kGrpT;
+constexpr int kStrStages = 6;
+constexpr size_t kStrHeaderBytes = 512;                                  // barriers + stage descriptors
 static_assert(kStatsPad >= 32 * (kGrpG + 2) + kGrpS + 1, "the widest (last) pass may read 32*(G+2)+S cells past the last t0 cell");
-static_assert(kStatsPad >= 32 * kFoldR, "a pass may read 32*R cells past the last t0 cell");
 
 struct PeriodicParams {
     const float2 *stats;             // [n_lc][n_dur][stats_pitch] (S_wmm, S_wmf), zero in null cells / padding
     const double *periods;           // [n_per] device
+    const double *r_cells;           // [n_per] device: periods[k] / t0_stride (IEEE FP64 division, done once on the host)
     const int *dur_lo, *dur_hi;      // [n_per] device or null
     unsigned long long *keys;        // [n_lc][n_per] packed (lr bits << 32 | ~cell id), 0 = no candidate
     unsigned int *counter;           // work-unit queue head
@@ -33,9 +36,10 @@ struct PeriodicParams {
 
 struct PeriodicPlan {
     PeriodicParams P{};
-    bool row_in_smem = false;        // grouped kernel (row in shared memory) or per-period kernel (row in L2)
+    bool row_in_smem = false;        // resident-row kernel (row in shared memory) or streamed kernel (row in L2)
     size_t smem_bytes = 0;
     int grid = 0;
+    int stage_cells = 0;             // streamed kernel: cells per ring stage
 };
 
 int build_periodic_plan(int32_t n_lc, int32_t n_dur, cetra_t0_grid grid, const double *durations_host,
@@ -45,6 +49,8 @@ size_t periodic_workspace_bytes(int32_t n_lc, int32_t n_per);   // periods, rang
 int run_periodic(PeriodicPlan &pl, const float2 *stats_dev, const double *periods_host, const int32_t *dur_lo_host,
                  const int32_t *dur_hi_host, bool upload, cetra_peak *peaks_dev, void *workspace_dev,
                  cudaStream_t st);
+int launch_fold_stream(const PeriodicPlan &pl, cudaStream_t st);   // fold_stream.cu
+int launch_fold_pair(const PeriodicPlan &pl, cudaStream_t st);     // fold_pair.cu
 int run_grids_to_stats(const float *depth_dev, const float *var_dev, int32_t n_rows, int64_t n_t0,
                        float2 *stats_dev, cudaStream_t st);
 
