@@ -81,22 +81,23 @@ __device__ __forceinline__ int consume_pass(StreamSmem *sm, uint32_t ring_addr, 
 #pragma unroll
         for (int g = 0; g < G; ++g) acc[t][g] = make_float2(0.f, 0.f);
     const int p0 = d.p0;
-    const long long limit = static_cast<long long>(n_t0) - 1 - p0;    // off_e <= limit  <=>  p0 + off_e <= I-1
+    const int limit = n_t0 - 1 - p0;                  // off_e <= limit  <=>  p0 + off_e <= I-1
     int flags;
     for (;;) {
-        const uint32_t slot = n_stage % kStrStages;
+        const uint32_t slot = (n_stage & (kStrStages - 1));
         flags = d.flags;
         if (wu.active) {
             // P1: the epoch's offsets of the two periods (FP64, R11); warp-uniform
             const double e = static_cast<double>(d.e);
-            const long long o0 = __double2ll_rn(__dmul_rn(e, wu.gp.r[0]));
-            const long long o1 = __double2ll_rn(__dmul_rn(e, wu.gp.r[1]));
+            // round-to-nearest-even conversion (= llrint for every in-range value), saturating
+            const int o0 = __double2int_rn(__dmul_rn(e, wu.gp.r[0]));
+            const int o1 = __double2int_rn(__dmul_rn(e, wu.gp.r[1]));
             if (o0 <= limit) {
                 if (!(flags & kDirect)) {
                     const uint32_t ptr = ring_addr + slot * stage_bytes +
-                                         8u * static_cast<uint32_t>(p0 + static_cast<int>(o0) - d.origin + lane * G);
-                    const long long dd = o1 - o0;
-                    switch (dd < 8 ? static_cast<int>(dd) : 8) {
+                                         8u * static_cast<uint32_t>(p0 + o0 - d.origin + lane * G);
+                    const int dd = o1 - o0;
+                    switch (dd < 8 ? dd : 8) {
                         case 0: fold_epoch<0, G>(acc, ptr); break;
                         case 1: fold_epoch<1, G>(acc, ptr); break;
                         case 2: fold_epoch<2, G>(acc, ptr); break;
@@ -132,23 +133,34 @@ __device__ __forceinline__ int consume_pass(StreamSmem *sm, uint32_t ring_addr, 
         if (lane == 0) mbar_arrive(&sm->empty[slot]);
         ++n_stage;
         if (flags & kLastOfPass) break;
-        const uint32_t nslot = n_stage % kStrStages;
-        mbar_wait(&sm->full[nslot], (n_stage / kStrStages) & 1u);
+        const uint32_t nslot = (n_stage & (kStrStages - 1));
+        mbar_wait(&sm->full[nslot], (n_stage >> kStrStagesLog2) & 1u);
         const int4 a = *reinterpret_cast<const int4 *>(&sm->desc[nslot]);
         d.origin = a.x; d.p0 = a.y; d.e = a.z; d.flags = a.w;
     }
-    // P3 + P4 within the lane: phases ascending, strict > keeps the smallest phase on ties
+    // P3 + P4 within the lane: phases ascending, strict > keeps the smallest phase on ties.  LR > best  <=>
+    // SB^2 > 2 best SA: cells that cannot beat the best so far are dismissed with that product (with a margin, so
+    // that none is dismissed wrongly); only when some cell of the lane passes does the lane take the divisions.
     if (wu.active) {
 #pragma unroll
         for (int t = 0; t < kGrpT; ++t) {
+            const float thr0 = 1.9999981f * wu.best_lr[t];
+            bool any = false;
 #pragma unroll
             for (int g = 0; g < G; ++g) {
-                const int p = p0 + lane * G + g;
-                const float a = acc[t][g].x, bsum = acc[t][g].y;
-                const float lr = 0.5f * bsum * bsum * rcp_approx(a);
-                if (p < wu.gp.n_phase[t] && a >= 1.17549435e-38f && lr > wu.best_lr[t]) {
-                    wu.best_lr[t] = lr;
-                    wu.best_p[t] = p;
+                const float2 pr = mul2(acc[t][g], make_float2(thr0, acc[t][g].y));   // (2 best SA, SB^2)
+                any |= pr.y >= pr.x;
+            }
+            if (any) {
+#pragma unroll
+                for (int g = 0; g < G; ++g) {
+                    const int p = p0 + lane * G + g;
+                    const float a = acc[t][g].x, bsum = acc[t][g].y;
+                    const float lr = 0.5f * bsum * bsum * rcp_approx(a);
+                    if (p < wu.gp.n_phase[t] && a >= 1.17549435e-38f && lr > wu.best_lr[t]) {
+                        wu.best_lr[t] = lr;
+                        wu.best_p[t] = p;
+                    }
                 }
             }
         }
@@ -176,36 +188,39 @@ __device__ __forceinline__ void begin_unit(const PeriodicParams &P, long long u,
         wu.gp.r[t] = r;
         wu.gp.n_phase[t] = on ? n_phase : 0;
         wu.kk[t] = k;
-        wu.best_lr[t] = -1.f;
+        // the period's best so far (rows already folded, by any CTA) only filters: a cell that ties it still passes
+        // (bits - 1) and the packed key decides ties by cell id, so the records do not depend on the fold order
+        const unsigned int hi = static_cast<unsigned int>(
+            *reinterpret_cast<volatile unsigned long long *>(P.keys + wu.lc * P.n_per + k) >> 32);
+        wu.best_lr[t] = hi ? __uint_as_float(hi - 1u) : -1.f;
         wu.best_p[t] = 0x7fffffff;
     }
     if (wu.gp.r[0] > wu.gp.r[1]) {                                 // sorted by ascending r
         const double tr = wu.gp.r[0]; wu.gp.r[0] = wu.gp.r[1]; wu.gp.r[1] = tr;
         const int tn = wu.gp.n_phase[0]; wu.gp.n_phase[0] = wu.gp.n_phase[1]; wu.gp.n_phase[1] = tn;
         const int tk = wu.kk[0]; wu.kk[0] = wu.kk[1]; wu.kk[1] = tk;
+        const float tb = wu.best_lr[0]; wu.best_lr[0] = wu.best_lr[1]; wu.best_lr[1] = tb;
     }
     wu.active = wu.gp.n_phase[0] > 0 || wu.gp.n_phase[1] > 0;
 }
 
 __device__ __forceinline__ void end_unit(const PeriodicParams &P, WarpUnit &wu, int lane) {
     if (!wu.active) return;
-    // P4 across the warp: larger lr wins, ties -> smaller phase; one atomicMax per period
+    // P4 across the warp: larger lr wins, ties -> smaller phase; one atomicMax per period (LR >= 0: its bit pattern
+    // orders like an unsigned integer)
 #pragma unroll
     for (int t = 0; t < kGrpT; ++t) {
-        float lr = wu.best_lr[t];
-        int p = wu.best_p[t];
-#pragma unroll
-        for (int s = 16; s > 0; s >>= 1) {
-            const float o_lr = __shfl_xor_sync(0xffffffffu, lr, s);
-            const int o_p = __shfl_xor_sync(0xffffffffu, p, s);
-            if (o_lr > lr || (o_lr == lr && o_p < p)) { lr = o_lr; p = o_p; }
-        }
-        if (lane == 0 && lr >= 0.f) {
-            const unsigned int id = static_cast<unsigned int>(wu.j) * static_cast<unsigned int>(P.n_t0) +
-                                    static_cast<unsigned int>(p);
-            const unsigned long long key =
-                (static_cast<unsigned long long>(__float_as_uint(lr)) << 32) | (0xffffffffu - id);
-            atomicMax(P.keys + wu.lc * P.n_per + wu.kk[t], key);
+        const bool has = wu.best_p[t] != 0x7fffffff;
+        if (__any_sync(0xffffffffu, has)) {
+            const unsigned int bits = has ? __float_as_uint(wu.best_lr[t]) : 0u;
+            const unsigned int top = __reduce_max_sync(0xffffffffu, bits);
+            const unsigned int p = __reduce_min_sync(
+                0xffffffffu, has && bits == top ? static_cast<unsigned int>(wu.best_p[t]) : 0x7fffffffu);
+            if (lane == 0) {
+                const unsigned int id = static_cast<unsigned int>(wu.j) * static_cast<unsigned int>(P.n_t0) + p;
+                const unsigned long long key = (static_cast<unsigned long long>(top) << 32) | (0xffffffffu - id);
+                atomicMax(P.keys + wu.lc * P.n_per + wu.kk[t], key);
+            }
         }
     }
 }
@@ -245,8 +260,8 @@ __global__ void __launch_bounds__(kStrThreads, 1) fold_stream_argmax_kernel(cons
         // ---------------- producer warp: claims units, derives every (pass, epoch) window, fills the ring
         uint32_t n_stage = 0;
         auto push = [&](const StageDesc &d, const float2 *src, uint32_t cells) {    // lane 0 only
-            const uint32_t slot = n_stage % kStrStages;
-            mbar_wait(&sm->empty[slot], ((n_stage / kStrStages) & 1u) ^ 1u);
+            const uint32_t slot = (n_stage & (kStrStages - 1));
+            mbar_wait(&sm->empty[slot], ((n_stage >> kStrStagesLog2) & 1u) ^ 1u);
             sm->desc[slot] = d;
             if (cells) {
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the stage was read by generic loads
@@ -369,8 +384,8 @@ __global__ void __launch_bounds__(kStrThreads, 1) fold_stream_argmax_kernel(cons
     wu.active = false;
     uint32_t n_stage = 0;
     for (;;) {
-        const uint32_t slot = n_stage % kStrStages;
-        mbar_wait(&sm->full[slot], (n_stage / kStrStages) & 1u);
+        const uint32_t slot = (n_stage & (kStrStages - 1));
+        mbar_wait(&sm->full[slot], (n_stage >> kStrStagesLog2) & 1u);
         const int4 a = *reinterpret_cast<const int4 *>(&sm->desc[slot]);
         const int4 b = *(reinterpret_cast<const int4 *>(&sm->desc[slot]) + 1);
         StageDesc d;

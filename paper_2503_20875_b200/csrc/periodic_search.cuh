@@ -15,7 +15,8 @@ constexpr size_t kGrpHeaderBytes = 16 + (kGrpThreads / 32) * 64 * 8;   // barrie
 // (640 threads keep the 96-register budget the two-period register window needs).
 constexpr int kStrThreads = 640;
 constexpr int kStrUnitPeriods = (kStrThreads / 32 - 1) * kGrpT;
-constexpr int kStrStages = 6;
+constexpr int kStrStagesLog2 = 3;
+constexpr int kStrStages = 1 << kStrStagesLog2;
 constexpr size_t kStrHeaderBytes = 512;                                  // barriers + stage descriptors
 static_assert(kStatsPad >= 32 * (kGrpG + 2) + kGrpS + 1, "the widest (last) pass may read 32*(G+2)+S cells past the last t0 cell");
 
