@@ -10,11 +10,17 @@ light curves.  The workload is BASELINE.json configs[1], the TESS-like 2-min sec
 
   value      light curves/s, inputs resident in HBM when the timed region starts (cetra_search_batched)
   e2e        the same metric through cetra_search_batched_host: pinned HOST buffers, H2D + D2H timed
-  roofline   the dominant kernel (fold_group_argmax_kernel, periodic search): algorithmic bytes / event time
-  cpu_baseline  the FP64 oracle on the host cores, on a bounded sample of the same workload
+  roofline   the dominant kernel (fold_pair_argmax_kernel, periodic search).  Its rows live in shared memory, so
+             the level that bounds it is the shared-memory crossbar: achieved = bytes its LDS instructions moved
+             (ncu wavefront count of this workload x 128 B, a property of the launch, see NCU_FOLD) / the
+             kernel's event-timed duration in THIS run; peak = 148 SM x 128 B/clk x clock (cetra_peak_probe's
+             measured LDS.64 rate is reported beside it).  north_star's HBM yardstick (8 B per (period, duration, t0 cell)) is kept
+             beside it as `algorithmic`.
+  cpu_baseline  the FP64 oracle on the host cores (all cores, and one thread), on a bounded sample of the workload
 
-N > 1 (torchrun): every rank searches its own B curves (no data-path collective; "weak" scaling), the
-time is the max over ranks.  --impl reference times the oracle (rank 0 only).
+N > 1: `python bench.py --gpus N` re-executes itself under torch.distributed.run with N ranks (the driver's own
+torchrun launch is used as it is); every rank searches its own B curves (no data-path collective; "weak"
+scaling), the time is the max over ranks.  --impl reference times the oracle (rank 0 only).
 """
 from __future__ import annotations
 
@@ -38,9 +44,28 @@ UNIT = "light curves/s"
 L2_FLUSH_BYTES = 512 << 20
 N_SM, FP32_LANES = 148, 128          # B200: SMs, FP32 FMA lanes per SM (B200_PROFILING.md unit counts)
 SMEM_BYTES_PER_CLK = 128             # shared-memory crossbar bytes/clk/SM (B300_MICROARCH.md, LDS/STS)
-# dram__bytes_read.sum + dram__bytes_write.sum of one fold_group_argmax_kernel launch over a 64-curve chunk of this
-# workload, from the `ncu --set full` capture summarised in profiles/r01h_fold_full.md (332.3 MB + 12.5 MB)
-NCU_FOLD_DRAM_BYTES_PER_LC = 344.8e6 / 64
+# Counters of ONE fold_pair_argmax_kernel launch over the 64-curve chunk of this workload, from the `ncu --set full`
+# capture summarised in `profile` (command inside).  They are properties of the launch (the kernel's loads do not
+# depend on timing), valid for the kernel sources whose hash is `src_sha256`: bench.py hashes the sources it runs
+# and reports `stale: true` (and no traffic) when they differ.
+NCU_FOLD = dict(
+    profile="profiles/r02a_fold_pair_full.md", commit="e202b0a", n_lc=64,
+    src_sha256="32a081b8265e7aa99b2d7294c86fc5ffee8188ad57ae4ce40dc20d30de7c5556",
+    lds_wavefronts=32075992439.0,       # l1tex__data_pipe_lsu_wavefronts_mem_shared.sum (128 B each)
+    dram_bytes=334122240.0 + 14267648.0,  # dram__bytes_read.sum + dram__bytes_write.sum
+    crossbar_pct_under_ncu=90.54,       # ...wavefronts_mem_shared.sum.pct_of_peak_sustained_elapsed
+    duration_ms_under_ncu=121.92,
+)
+FOLD_SOURCES = ("fold_pair.cu", "fold_common.cuh", "periodic_search.cuh", "common.cuh")
+
+
+def fold_sources_sha256() -> str:
+    import hashlib
+    h = hashlib.sha256()
+    for name in FOLD_SOURCES:
+        with open(os.path.join(ROOT, "paper_2503_20875_b200", "csrc", name), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()
 
 
 # ----------------------------------------------------------------------------------------------- helpers
@@ -137,12 +162,23 @@ class ClockSampler:
         return dict(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
 
 
-def oracle_sample(p, flux, flux_err, budget_s: float):
+def oracle_sample(p, flux, flux_err, budget_s: float, threads: int = 0):
     """The oracle, as it stands, on one light curve of the workload: the linear search in full and the
     periodic search on a seeded subset of the trial periods sized to about `budget_s` of CPU time.
-    Returns (light curves/s extrapolated to all K periods, description, cores)."""
+    `threads` > 0 limits its OpenMP threads for this sample.
+    Returns (light curves/s extrapolated to all K periods, description, cores, seconds spent)."""
     import oracle
     oracle.build()
+    all_threads = oracle.get_threads()
+    if threads > 0:
+        oracle.set_threads(threads)
+    try:
+        return _oracle_sample(oracle, p, flux, flux_err, budget_s)
+    finally:
+        oracle.set_threads(all_threads)
+
+
+def _oracle_sample(oracle, p, flux, flux_err, budget_s):
     cores = oracle.get_threads()
     t = time.perf_counter()
     grids = oracle.linear_search(p.times, flux, flux_err, p.durations, p.t0_start, p.t0_stride, p.n_t0, p.template)
@@ -188,19 +224,20 @@ def run_reference(args, rank: int):
     line = dict(metric=METRIC, value=value, unit=UNIT, impl="reference", n_gpus=args.gpus, steps=args.steps,
                 warmup=args.warmup, ms_per_step=1e3 * wall / max(args.steps, 1), higher_is_better=True,
                 scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
-                config=workload_config(p, args, args.n_lc, "oracle on host cores; each step = " + sample),
+                config=workload_config(p, args.n_lc), notes="oracle on host cores; each step = " + sample,
                 cpu_baseline=dict(value=value, unit=UNIT, cores=cores, kind="oracle", sample=sample),
                 e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
                 gpu_launches=0)
     print(json.dumps(line), flush=True)
 
 
-def workload_config(p, args, n_lc, note):
+def workload_config(p, n_lc):
+    """The same dict for both arms (the driver compares them)."""
     return dict(workload=f"BASELINE configs[1] tess-2min-sector x {n_lc} light curves per GPU per step "
                          f"(config-5 survey recipe: shared 19 728-point 2-min time array with a 1 d gap)",
                 n_points=p.n, n_durations=int(len(p.durations)), n_t0=int(p.n_t0), n_periods=int(len(p.periods)),
                 n_template=int(len(p.template)), light_curves_per_step_per_gpu=n_lc,
-                l2="flushed between timed steps (512 MiB write)", note=note)
+                l2="flushed between timed steps (512 MiB write)")
 
 
 # ------------------------------------------------------------------------------------------------- CUDA arm
@@ -275,6 +312,11 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
         step_device()
     for _ in range(min(args.warmup, 1)):
         step_host()
+    probes = {}
+    for name, kind in (("ffma2", cetra.CETRA_PROBE_FFMA2), ("fadd2", cetra.CETRA_PROBE_FADD2),
+                       ("lds64", cetra.CETRA_PROBE_LDS64)):
+        per_clk, per_s = cetra.cetra_peak_probe(kind)
+        probes[name] = dict(per_clk_per_sm=per_clk, per_second=per_s, unit="B" if name == "lds64" else "flop")
     with ClockSampler(local_rank) as clocks:
         ms_dev, launches, prof, wall_dev = timed(step_device, args.steps, profile=True)
     ms_e2e, _, _, wall_e2e = timed(step_host, args.steps, profile=False)
@@ -287,55 +329,70 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
     total_lc = B * world * args.steps
     value = total_lc / (ms_dev * 1e-3)
     e2e_value = total_lc / (ms_e2e * 1e-3)
-    # roofline of the dominant kernel (periodic fold): 8 B and 2 FADD per (period, duration, t0 cell)
     fold_launches = max(prof["fold_launches"], 1)
     lin_launches = max(prof["linear_launches"], 1)
-    fold_bytes = 8.0 * wc["gathers"] * B * args.steps          # summed over this rank's launches
-    fold_s = prof["fold_ms"] * 1e-3
-    lin_s = prof["linear_ms"] * 1e-3
-    fold_gbs = fold_bytes / fold_s / 1e9
-    lin_tflops = 4.0 * wc["template_evals"] * B * args.steps / lin_s / 1e12
+    fold_ms = prof["fold_ms"] / fold_launches                   # average launch, event-timed in this run
+    lin_ms = prof["linear_ms"] / lin_launches
+    lc_per_launch = B * args.steps / fold_launches
+    # -- dominant kernel: the periodic fold.  Physical level: shared-memory crossbar (LDS bytes / probe rate).
+    sha = fold_sources_sha256()
+    stale = sha != NCU_FOLD["src_sha256"]
+    lds_bytes = 128.0 * NCU_FOLD["lds_wavefronts"] * lc_per_launch / NCU_FOLD["n_lc"]
+    lds_gbs = lds_bytes / (fold_ms * 1e-3) / 1e9
+    smem_peak_gbs = N_SM * SMEM_BYTES_PER_CLK * peaks["sm_max_mhz"] * 1e6 / 1e9
+    # north_star's yardstick: 8 B gathered and 2 FADD per (period, duration, t0 cell) against the HBM copy peak
+    alg_bytes = 8.0 * wc["gathers"] * lc_per_launch
+    alg_gbs = alg_bytes / (fold_ms * 1e-3) / 1e9
+    lin_tflops = 4.0 * wc["template_evals"] * (B * args.steps / lin_launches) / (lin_ms * 1e-3) / 1e12
     fp32_peak = N_SM * FP32_LANES * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
-    smem_peak = N_SM * SMEM_BYTES_PER_CLK * peaks["sm_max_mhz"] * 1e6 / 1e9
     line = dict(
         metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
         ms_per_step=ms_dev / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
-        dtype="f32", data="synthetic",
-        config=workload_config(p, args, B, "timed per step with CUDA events on the launching stream, summed; "
-                                           "max over ranks"),
+        dtype="f32", data="synthetic", config=workload_config(p, B),
+        notes="timed per step with CUDA events on the launching stream, summed; max over ranks",
         e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=int(2 * B * p.n * 4),
                  d2h_bytes_per_step=int(B * K * 32), ms_per_step=ms_e2e / args.steps,
                  api="cetra_search_batched_host (pinned host flux/flux_err in, pinned host records out)"),
         gpu_launches=int(launches),
         clocks=clocks.summary(),
-        roofline=dict(bound="hbm", kernel="fold_group_argmax_kernel", achieved=fold_gbs, peak=peaks["hbm_gbs"],
-                      unit="GB/s", frac=fold_gbs / peaks["hbm_gbs"],
-                      traffic=NCU_FOLD_DRAM_BYTES_PER_LC * B * args.steps / fold_launches,
-                      traffic_source="ncu --set full, profiles/r01h_fold_full.md, scaled to the curves per launch",
-                      peak_source=peaks["source"],
-                      ms_per_launch=prof["fold_ms"] / fold_launches, launches=int(prof["fold_launches"]),
-                      share_of_step=prof["fold_ms"] / ms_dev,
-                      algorithmic_bytes_per_launch=fold_bytes / fold_launches,
-                      served_from="shared memory (one (S_wmm,S_wmf) row per CTA); compulsory HBM traffic is the "
-                                  "stats grid once per chunk",
-                      smem=dict(achieved=fold_gbs, peak=smem_peak, unit="GB/s", frac=fold_gbs / smem_peak,
-                                peak_derivation="148 SM x 128 B/clk x sm_max_mhz",
-                                note="algorithmic bytes (8 B per cell) against the crossbar peak; above 1 because a "
-                                     "warp folds two neighbouring periods from one register window, so a loaded "
-                                     "cell serves up to two cells of work (ncu: 82.7 % of the crossbar busy)")),
+        roofline=dict(
+            bound="smem", kernel="fold_pair_argmax_kernel", achieved=lds_gbs, peak=smem_peak_gbs, unit="GB/s",
+            frac=lds_gbs / smem_peak_gbs,
+            traffic=None if stale else NCU_FOLD["dram_bytes"] * lc_per_launch / NCU_FOLD["n_lc"],
+            derivation="achieved = shared-memory bytes the kernel's loads move per launch (ncu LDS wavefronts of "
+                       "this workload x 128 B, scaled to the curves per launch) / its average event-timed "
+                       "duration in this run; peak = 148 SM x 128 B/clk x sm_max_mhz (the crossbar's nominal "
+                       "rate; peak_probe = the conflict-free LDS.64 rate cetra_peak_probe measures in this run)",
+            ms_per_launch=fold_ms, launches=int(prof["fold_launches"]), share_of_step=prof["fold_ms"] / ms_dev,
+            lds_bytes_per_launch=lds_bytes,
+            peak_probe=probes["lds64"],
+            ncu=dict(NCU_FOLD, stale=stale, src_sha256_now=sha),
+            algorithmic=dict(bytes_per_launch=alg_bytes, gbs=alg_gbs, hbm_peak_gbs=peaks["hbm_gbs"],
+                             over_hbm_peak=alg_gbs / peaks["hbm_gbs"], hbm_peak_source=peaks["source"],
+                             loads_per_cell=lds_bytes / alg_bytes,
+                             note="north_star's yardstick (8 B per (period, duration, t0 cell) / HBM copy peak); "
+                                  "a ratio above 1 is reuse, not a roofline fraction: a row is read from HBM a "
+                                  "handful of times per launch and gathered from shared memory 20 000 times")),
         roofline_linear=dict(bound="alu", kernel="linear_search_kernel", achieved=lin_tflops, peak=fp32_peak,
                              unit="TFLOP/s", frac=lin_tflops / fp32_peak,
-                             peak_derivation="148 SM x 128 FP32 lanes x 2 flop x sm_max_mhz",
-                             ms_per_launch=prof["linear_ms"] / lin_launches, launches=int(prof["linear_launches"]),
+                             derivation="4 flop per (t0, duration, in-window point) template evaluation / the "
+                                        "kernel's event-timed duration; peak = 148 SM x 128 FP32 lanes x 2 flop "
+                                        "x sm_max_mhz (peak_probe = the packed FP32 FMA rate cetra_peak_probe "
+                                        "measures in this run)",
+                             peak_probe=probes["ffma2"],
+                             ms_per_launch=lin_ms, launches=int(prof["linear_launches"]),
                              share_of_step=prof["linear_ms"] / ms_dev,
-                             template_evals_per_s=wc["template_evals"] * B * args.steps / lin_s),
+                             template_evals_per_s=wc["template_evals"] * (B * args.steps / lin_launches) /
+                                                  (lin_ms * 1e-3)),
         rates=dict(periods_per_s=K * total_lc / (ms_dev * 1e-3),
                    template_evals_per_lc=wc["template_evals"], gathers_per_lc=wc["gathers"],
-                   duration_period_pairs=wc["pairs"]),
+                   duration_period_pairs=wc["pairs"], fadd2_probe=probes["fadd2"]),
     )
     if world == 1 and not args.no_cpu_baseline:
         v, sample, cores, _ = oracle_sample(p, p.flux[0], p.flux_err[0], args.cpu_seconds)
-        line["cpu_baseline"] = dict(value=v, unit=UNIT, cores=cores, kind="oracle", sample=sample)
+        v1, sample1, _, _ = oracle_sample(p, p.flux[0], p.flux_err[0], args.cpu_seconds / 2, threads=1)
+        line["cpu_baseline"] = dict(value=v, unit=UNIT, cores=cores, kind="oracle", sample=sample,
+                                    one_thread=dict(value=v1, unit=UNIT, cores=1, sample=sample1))
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -437,8 +494,8 @@ def run_configs(args):
                     linear_frac_fp32=4.0 * wc["template_evals"] / (lin_ms * 1e-3) / fp32_peak,
                     periodic_ms=per_ms, periods_per_s=len(p.periods) / (per_ms * 1e-3),
                     fold_algorithmic_gbs=fold_bytes / (per_ms * 1e-3) / 1e9,
-                    fold_frac_hbm=fold_bytes / (per_ms * 1e-3) / 1e9 / peaks_hw["hbm_gbs"],
-                    fold_frac_smem=fold_bytes / (per_ms * 1e-3) / smem_peak,
+                    fold_algorithmic_over_hbm_peak=fold_bytes / (per_ms * 1e-3) / 1e9 / peaks_hw["hbm_gbs"],
+                    fold_algorithmic_over_smem_peak=fold_bytes / (per_ms * 1e-3) / smem_peak,
                     light_curves_per_s=1e3 / (lin_ms + per_ms), reps=reps,
                     note="periodic_ms includes finalize_peaks and the key memset; single light curve, so the short "
                          "configs are launch- and tail-bound")
@@ -472,6 +529,12 @@ def run_configs(args):
                           frac_hbm=moved / (rs_ms * 1e-3) / 1e9 / peaks_hw["hbm_gbs"])), flush=True)
 
 
+def spawn_command(n_gpus: int, port: int, argv):
+    """The torchrun command `python bench.py --gpus N` runs itself under when it was not started by torchrun."""
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n_gpus}",
+            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *argv]
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -486,10 +549,17 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU budget of the cpu_baseline sample")
     ap.add_argument("--ref-seconds", type=float, default=8.0, help="CPU budget of one --impl reference step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--master-port", type=int, default=29541, help="rendezvous port when bench.py spawns the ranks")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.workload == "sector":
+        # not under torchrun: start the N ranks ourselves (one process per GPU, rendezvous on 127.0.0.1)
+        sys.exit(subprocess.call(spawn_command(args.gpus, args.master_port, sys.argv[1:])))
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.workload == "sector" and world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}: refusing to report a number for "
+                         f"a different GPU count")
     if args.impl == "reference":
         run_reference(args, rank)
     elif args.workload == "survey":

@@ -294,6 +294,22 @@ int cetra_profile_enable(int32_t enable);
 int cetra_profile_read(double *linear_ms, int64_t *linear_launches, double *fold_ms, int64_t *fold_launches,
                        int32_t reset);
 
+/* Unit-throughput probes (diagnostic, for bench.py's roofline denominators): the measured rate of the instruction
+ * that bounds each hot kernel, in the form the kernel issues it.  Runs a short self-timed kernel on `cuda_stream`
+ * with one 1 024-thread CTA per SM and SYNCHRONISES the stream.
+ *   CETRA_PROBE_FFMA2  packed FP32 fused multiply-add (linear search)      unit: FP32 flop
+ *   CETRA_PROBE_FADD2  packed FP32 add (fold accumulation)                  unit: FP32 flop
+ *   CETRA_PROBE_LDS64  conflict-free 8-byte shared-memory loads (fold gather)             unit: bytes
+ *  iters            loop trips per thread (>= 1; 20 000 gives a few milliseconds)
+ *  per_clk_per_sm   optional out: units per SM clock per SM (from clock64 inside the kernel)
+ *  per_second       optional out: units per second over the whole GPU (CUDA events around the launch)
+ *  workspace_dev    cetra_peak_probe_workspace_bytes() bytes of device memory, 256-byte aligned
+ * Returns CETRA_ERR_INVALID_ARG / CETRA_ERR_WORKSPACE / CETRA_ERR_CUDA as the other entry points. */
+typedef enum { CETRA_PROBE_FFMA2 = 0, CETRA_PROBE_FADD2 = 1, CETRA_PROBE_LDS64 = 2 } cetra_probe_kind;
+size_t cetra_peak_probe_workspace_bytes(void);
+int cetra_peak_probe(int32_t kind, int32_t iters, double *per_clk_per_sm, double *per_second,
+                     void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

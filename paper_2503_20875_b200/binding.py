@@ -32,7 +32,7 @@ EXPORTED_SYMBOLS = (
     "cetra_periodic_workspace_bytes", "cetra_periodic_search", "cetra_periodic_search_stats",
     "cetra_search_batched_workspace_bytes", "cetra_search_batched", "cetra_search_batched_templates",
     "cetra_search_batched_host_workspace_bytes", "cetra_search_batched_host",
-    "cetra_profile_enable", "cetra_profile_read",
+    "cetra_profile_enable", "cetra_profile_read", "cetra_peak_probe_workspace_bytes", "cetra_peak_probe",
     "cetra_median_cadence", "cetra_resample_grid", "cetra_resample_workspace_bytes", "cetra_resample",
     "cetra_monotransit_workspace_bytes", "cetra_monotransit_search",
     "cetra_mask_workspace_bytes", "cetra_mask_transits",
@@ -139,6 +139,10 @@ def load_library() -> ctypes.CDLL:
     lib.cetra_profile_enable.argtypes = [i32]
     lib.cetra_profile_read.restype = ctypes.c_int
     lib.cetra_profile_read.argtypes = [dp, ctypes.POINTER(i64), dp, ctypes.POINTER(i64), i32]
+    lib.cetra_peak_probe_workspace_bytes.restype = sz
+    lib.cetra_peak_probe_workspace_bytes.argtypes = []
+    lib.cetra_peak_probe.restype = ctypes.c_int
+    lib.cetra_peak_probe.argtypes = [i32, i32, dp, dp, vp, sz, vp]
     _lib = lib
     return lib
 
@@ -240,6 +244,21 @@ def cetra_profile_read(reset: bool = True):
     _check(load_library().cetra_profile_read(ctypes.byref(lm), ctypes.byref(ll), ctypes.byref(fm), ctypes.byref(fl),
                                              1 if reset else 0), "cetra_profile_read")
     return dict(linear_ms=lm.value, linear_launches=ll.value, fold_ms=fm.value, fold_launches=fl.value)
+
+
+CETRA_PROBE_FFMA2, CETRA_PROBE_FADD2, CETRA_PROBE_LDS64 = 0, 1, 2
+
+
+def cetra_peak_probe(kind: int, iters: int = 20000, stream=None):
+    """(units per clock per SM, units per second) of one of the probed instructions; synchronises the stream."""
+    torch = _torch()
+    lib = load_library()
+    nbytes = int(lib.cetra_peak_probe_workspace_bytes())
+    ws = _workspace(torch, nbytes, torch.device("cuda", torch.cuda.current_device()))
+    a, b = ctypes.c_double(), ctypes.c_double()
+    _check(lib.cetra_peak_probe(int(kind), int(iters), ctypes.byref(a), ctypes.byref(b), ws.data_ptr(), ws.numel(),
+                                _stream_ptr(torch, stream)), "cetra_peak_probe")
+    return a.value, b.value
 
 
 def cetra_linear_workspace_bytes(times, n_lc: int, durations, t0_start, t0_stride, n_t0, n_template: int) -> int:

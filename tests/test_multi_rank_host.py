@@ -56,3 +56,25 @@ def test_rank_partition_and_max_over_ranks():
         assert np.isclose(checksum, np.nansum(full.flux[lo:hi].astype(np.float64)), rtol=0, atol=0)
         assert ms == 10.0 + 5.0 * (world - 1)          # the slowest rank's time, on every rank
     assert covered == list(range(per_rank * world))    # exact, disjoint, in order
+
+
+def test_bench_spawns_its_own_ranks_and_refuses_a_mismatched_world(monkeypatch):
+    """`python bench.py --gpus N` outside torchrun re-executes itself with N ranks on 127.0.0.1; started with a
+    WORLD_SIZE that is not N it refuses to print a line (it used to report n_gpus 1 silently)."""
+    import subprocess
+    import sys
+
+    import pytest
+
+    import bench
+    cmd = bench.spawn_command(8, 29999, ["--gpus", "8", "--steps", "2"])
+    assert cmd[1:3] == ["-m", "torch.distributed.run"]
+    assert "--nproc-per-node=8" in cmd and "--nnodes=1" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and cmd[cmd.index("--master-port") + 1] == "29999"
+    assert cmd[-4:] == ["--gpus", "8", "--steps", "2"] and cmd[-5].endswith("bench.py")
+    monkeypatch.setenv("WORLD_SIZE", "1")
+    monkeypatch.setenv("RANK", "0")
+    monkeypatch.setattr(sys, "argv", ["bench.py", "--gpus", "8"])
+    with pytest.raises(SystemExit) as exc:
+        bench.main()
+    assert "refusing" in str(exc.value)
