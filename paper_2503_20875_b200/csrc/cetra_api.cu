@@ -264,7 +264,8 @@ int32_t default_chunk(int32_t n_lc, int32_t n_dur, int64_t n_t0) {
     const size_t per_lc = sizeof(float2) * static_cast<size_t>(n_dur) * static_cast<size_t>(cetra_stats_pitch(n_t0));
     const size_t budget = 512ull << 20;
     const size_t c = std::max<size_t>(1, budget / std::max<size_t>(per_lc, 1));
-    return static_cast<int32_t>(std::min<size_t>(c, static_cast<size_t>(n_lc)));
+    // (65 535: light curves are the z dimension of the linear kernels' grids)
+    return static_cast<int32_t>(std::min<size_t>(std::min<size_t>(c, 65535), static_cast<size_t>(n_lc)));
 }
 
 int plan_batched(const double *times_host, int64_t n, int32_t n_lc, int32_t lc_chunk, const double *durations_host,

@@ -116,11 +116,10 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
     constexpr int TILE = WARPS * 32 * R;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
-    const int per_lc = P.tiles_per_row * P.n_dur;
-    const long long lc = blockIdx.x / per_lc;
-    const int rem = static_cast<int>(blockIdx.x - lc * per_lc);
-    const int j = P.order[rem / P.tiles_per_row];               // longest durations first
-    const int tile = rem % P.tiles_per_row;
+    // grid = (tiles of a row, durations, light curves): consecutive blocks share a duration's tap table
+    const long long lc = blockIdx.z;
+    const int j = P.order[blockIdx.y];                          // longest durations first
+    const int tile = blockIdx.x;
     const int q = P.q;
     const int A = P.A[j];
     const long long i_blk = static_cast<long long>(tile) * TILE;
@@ -138,7 +137,8 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
     // branch b reads stream v = (e0 + b) mod q from position (e0 + b) div q + i_blk on
     auto issue = [&](int b, bool with_taps) {
         const unsigned int e = e0 + static_cast<unsigned int>(b);
-        const long long v = e % uq, u0 = e / uq + i_blk;
+        const unsigned int eu = q == 1 ? e : e / uq;
+        const long long v = e - eu * uq, u0 = eu + i_blk;
         const int d0 = static_cast<int>(u0 & 1);                 // bulk copies need 16-byte alignment
         const uint32_t bytes = static_cast<uint32_t>(slice) * 8u;
         const uint32_t bytes_taps = with_taps ? static_cast<uint32_t>(n_tap) * 8u : 0u;
@@ -177,7 +177,8 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
     for (int b = 0; b < q; ++b) {
         if (tid == 0 && b + 1 < q) issue(b + 1, false);          // its stage was released at the end of branch b-1
         mbar_wait(bar + (b & 1), static_cast<uint32_t>((b >> 1) & 1));
-        const int d0 = static_cast<int>(((e0 + static_cast<unsigned int>(b)) / uq + i_blk) & 1);
+        const unsigned int eb = e0 + static_cast<unsigned int>(b);
+        const int d0 = static_cast<int>(((q == 1 ? eb : eb / uq) + i_blk) & 1);
         const float2 *xb = stage0 + (b & 1) * slice + d0 + tid * R;
         const float2 *tb = taps + b * A;
         float2 win[R];
@@ -222,19 +223,33 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
     __syncwarp();
     const long long row = lc * P.n_dur + j;
     const long long i_warp = i_blk + static_cast<long long>(warp) * (32 * R);
+    const long long left_ll = P.n_t0 - i_warp - lane;           // cell r*32 + lane of the warp exists iff r*32 < left
+    const int left = left_ll > 32 * R ? 32 * R : static_cast<int>(left_ll);
+    const float2 *sl = st + lane;
+    if (P.stats) {                                               // the form the periodic search consumes: no division
+        float2 *out = P.stats + row * P.stats_pitch + i_warp + lane;
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const long long i = i_warp + r * 32 + lane;
-        if (i < P.n_t0) {
-            const float2 ab = st[r * 32 + lane];
-            const float a = ab.x, bsum = ab.y;
-            const bool null_cell = !(a > 0.f);                  // no observation in the window
-            const float nanv = __int_as_float(0x7fc00000);
-            const float depth = null_cell ? nanv : bsum / a;
-            if (P.depth) P.depth[row * P.n_t0 + i] = depth;
-            if (P.var) P.var[row * P.n_t0 + i] = null_cell ? nanv : 1.0f / a;
-            if (P.dlogL) P.dlogL[row * P.n_t0 + i] = null_cell ? nanv : 0.5f * bsum * depth;
-            if (P.stats) P.stats[row * P.stats_pitch + i] = null_cell ? make_float2(0.f, 0.f) : ab;
+        for (int r = 0; r < R; ++r) {
+            if (r * 32 < left) {
+                const float2 ab = sl[r * 32];
+                out[r * 32] = ab.x > 0.f ? ab : make_float2(0.f, 0.f);   // no observation in the window: null
+            }
+        }
+    }
+    if (P.depth || P.var || P.dlogL) {
+        const long long o = row * P.n_t0 + i_warp + lane;
+        const float nanv = __int_as_float(0x7fc00000);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            if (r * 32 < left) {
+                const float2 ab = sl[r * 32];
+                const float a = ab.x, bsum = ab.y;
+                const bool null_cell = !(a > 0.f);              // no observation in the window
+                const float depth = null_cell ? nanv : bsum / a;
+                if (P.depth) P.depth[o + r * 32] = depth;
+                if (P.var) P.var[o + r * 32] = null_cell ? nanv : 1.0f / a;
+                if (P.dlogL) P.dlogL[o + r * 32] = null_cell ? nanv : 0.5f * bsum * depth;
+            }
         }
     }
 }
@@ -339,7 +354,15 @@ int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const d
     for (int j = 0; j < n_dur; ++j) {
         const double D = durations_host[j];
         if (!(D > 0.0) || !std::isfinite(D)) return CETRA_ERR_INVALID_ARG;
-        const double h = floor(D / (2.0 * pl->geo.cadence)) + 1.0;     // safe superset of the window (R2)
+        // window half-reach in samples (R2): floor(D / 2c), one more where the taps' own rounded arithmetic
+        // (build_taps_kernel) still places sample h + 1 inside 0 <= x <= 1
+        double h = floor(D / (2.0 * pl->geo.cadence));
+        {
+            const volatile double kc = (h + 1.0) * pl->geo.cadence;
+            const volatile double xr = kc / D;
+            const volatile double x_hi = xr + 0.5, x_lo = -xr + 0.5;
+            if (x_hi <= 1.0 || x_lo >= 0.0) h += 1.0;
+        }
         if (h > 4.0e6) return CETRA_ERR_UNSUPPORTED;
         P.H[j] = static_cast<int>(h);
         const int ntap = 2 * P.H[j] + 1;
@@ -376,7 +399,7 @@ int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const d
     pl->warps = warps;
     pl->tile = warps * 32 * R;
     P.tiles_per_row = static_cast<int>((grid.n_t0 + pl->tile - 1) / pl->tile);
-    if (static_cast<long long>(P.tiles_per_row) * n_dur * n_lc > 0x7fffffffLL) return CETRA_ERR_UNSUPPORTED;
+    if (n_lc > 65535) return CETRA_ERR_UNSUPPORTED;          // light curves are the grid's z dimension
     pl->smem_bytes = linear_smem_bytes(*pl, R, warps);
 
     // padded (w f, w) samples in q polyphase streams: element u of stream v is sample n_lo + q u + v
@@ -397,10 +420,11 @@ size_t linear_workspace_bytes(const LinearPlan &pl, int32_t n_lc, int32_t n_temp
 }
 
 template <int R, int WARPS>
-static int launch_linear(const LinearPlan &pl, const LinearParams &P, long long blocks, cudaStream_t st) {
+static int launch_linear(const LinearPlan &pl, const LinearParams &P, int32_t n_lc, cudaStream_t st) {
     auto k = linear_search_kernel<R, WARPS>;
     CETRA_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes));
-    k<<<static_cast<unsigned>(blocks), WARPS * 32, pl.smem_bytes, st>>>(P);
+    const dim3 grid(static_cast<unsigned>(P.tiles_per_row), static_cast<unsigned>(P.n_dur), static_cast<unsigned>(n_lc));
+    k<<<grid, WARPS * 32, pl.smem_bytes, st>>>(P);
     CETRA_LAUNCH_CHECK();
     return CETRA_OK;
 }
@@ -468,14 +492,13 @@ int run_linear(LinearPlan &pl, const void *flux_dev, const void *flux_err_dev, c
         CETRA_LAUNCH_CHECK();
         return CETRA_OK;
     }
-    const long long blocks = static_cast<long long>(P.tiles_per_row) * P.n_dur * n_lc;
     constexpr int R = kLinearR;
     profile_mark(kProfLinear, true, st);
     int rc;
     switch (pl.warps) {
-        case 4: rc = launch_linear<R, 4>(pl, P, blocks, st); break;
-        case 2: rc = launch_linear<R, 2>(pl, P, blocks, st); break;
-        default: rc = launch_linear<R, 1>(pl, P, blocks, st); break;
+        case 4: rc = launch_linear<R, 4>(pl, P, n_lc, st); break;
+        case 2: rc = launch_linear<R, 2>(pl, P, n_lc, st); break;
+        default: rc = launch_linear<R, 1>(pl, P, n_lc, st); break;
     }
     profile_mark(kProfLinear, false, st);
     return rc;
