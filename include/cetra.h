@@ -113,6 +113,15 @@ int cetra_linear_search(const double *times_host, const void *flux_dev, const vo
                         float *depth_dev, float *var_dev, float *dlogL_dev, float *stats_dev,
                         void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
 
+/* t0 grids off the sample grid (the paper's default stride is 1 % of the shortest duration; DESIGN.md
+ * R25) are searched without evaluating the definition's FP64 expression for every (cell, sample) pair: the
+ * nearest-neighbour template sample is taken from a position computed once per residue class of cells (stride /
+ * cadence rational) or by fixed-point stepping (any stride), and only pairs whose position lies within a proven
+ * rounding bound of a decision point (an index step, a window edge) are evaluated with the exact R25 sequence, so the
+ * result is the definition's.  This diagnostic returns how many exact evaluations the device has done since the last
+ * reset.  Synchronises the device.  count may be NULL.  Returns CETRA_OK or CETRA_ERR_CUDA. */
+int cetra_exact_eval_count(int64_t *count, int32_t reset);
+
 /* Row pitch (in cells) of the sufficient-statistics grid for n_t0 cells. */
 int64_t cetra_stats_pitch(int64_t n_t0);
 

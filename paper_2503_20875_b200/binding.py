@@ -28,7 +28,7 @@ CETRA_MAX_DURATIONS = 128
 # Every symbol include/cetra.h declares (tests check that the library exports each of them).
 EXPORTED_SYMBOLS = (
     "cetra_status_string", "cetra_device_info", "cetra_stats_pitch", "cetra_kernel_launch_count",
-    "cetra_linear_workspace_bytes", "cetra_linear_search",
+    "cetra_linear_workspace_bytes", "cetra_linear_search", "cetra_exact_eval_count",
     "cetra_periodic_workspace_bytes", "cetra_periodic_search", "cetra_periodic_search_stats",
     "cetra_search_batched_workspace_bytes", "cetra_search_batched", "cetra_search_batched_templates",
     "cetra_search_batched_host_workspace_bytes", "cetra_search_batched_host",
@@ -92,6 +92,8 @@ def load_library() -> ctypes.CDLL:
     lib.cetra_stats_pitch.argtypes = [i64]
     lib.cetra_kernel_launch_count.restype = i64
     lib.cetra_kernel_launch_count.argtypes = []
+    lib.cetra_exact_eval_count.restype = ctypes.c_int
+    lib.cetra_exact_eval_count.argtypes = [ctypes.POINTER(i64), i32]
     lib.cetra_linear_workspace_bytes.restype = sz
     lib.cetra_linear_workspace_bytes.argtypes = [dp, i64, i32, dp, i32, cetra_t0_grid, i32]
     lib.cetra_linear_search.restype = ctypes.c_int
@@ -231,6 +233,13 @@ def cetra_stats_pitch(n_t0: int) -> int:
 
 def cetra_kernel_launch_count() -> int:
     return int(load_library().cetra_kernel_launch_count())
+
+
+def cetra_exact_eval_count(reset: bool = False) -> int:
+    """Exact (R25) evaluations done by the off-grid linear search since the last reset (synchronises)."""
+    v = ctypes.c_int64()
+    _check(load_library().cetra_exact_eval_count(ctypes.byref(v), 1 if reset else 0), "cetra_exact_eval_count")
+    return int(v.value)
 
 
 def cetra_profile_enable(enable: bool) -> None:

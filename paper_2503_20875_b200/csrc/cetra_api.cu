@@ -73,6 +73,36 @@ int derive_geometry(const double *times_host, int64_t n, cetra_t0_grid grid, Geo
     g->on_grid = !(drift > 1e-6 || ib < 1);
     g->n0 = g->on_grid ? ia : 0;
     g->q = g->on_grid ? ib : 0;
+    g->rational = false;
+    g->cls = 1;
+    g->drift = 0.0;
+    if (!g->on_grid) {
+        // continued-fraction convergents of stride / cadence with a denominator of at most kMaxClasses
+        long long p0 = 0, q0 = 1, p1 = 1, q1 = 0;
+        double x = b;
+        for (int it = 0; it < 40; ++it) {
+            const double fl = floor(x);
+            if (!(fl < 1e9)) break;
+            const long long ai = static_cast<long long>(fl);
+            const long long p2 = ai * p1 + p0, q2 = ai * q1 + q0;
+            if (q2 > kMaxClasses || p2 > kMaxClassStride) break;
+            p0 = p1; q0 = q1; p1 = p2; q1 = q2;
+            const double fr = x - fl;
+            if (fabs(b - static_cast<double>(p1) / static_cast<double>(q1)) * static_cast<double>(grid.n_t0) <= 1e-9 ||
+                !(fr > 1e-12))
+                break;
+            x = 1.0 / fr;
+        }
+        if (q1 >= 1 && p1 >= 1) {
+            const double dr = fabs(b - static_cast<double>(p1) / static_cast<double>(q1)) * static_cast<double>(grid.n_t0);
+            if (dr <= 1e-6) {
+                g->rational = true;
+                g->q = p1;
+                g->cls = q1;
+                g->drift = dr + 1e-12;
+            }
+        }
+    }
     return CETRA_OK;
 }
 
@@ -196,6 +226,12 @@ int cetra_linear_search(const double *times_host, const void *flux_dev, const vo
     if ((rc = require_device()) != CETRA_OK) return rc;
     return run_linear(pl, flux_dev, flux_err_dev, dtype, n, n_lc, template_host, n_template, false, depth_dev,
                       var_dev, dlogL_dev, stats_dev, workspace_dev, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int cetra_exact_eval_count(int64_t *count, int32_t reset) {
+    const int rc = require_device();
+    if (rc != CETRA_OK) return rc;
+    return exact_eval_count(count, reset != 0);
 }
 
 // ---------------------------------------------------------------------------------------- periodic

@@ -30,6 +30,8 @@ void profile_mark(ProfiledKernel which, bool begin, cudaStream_t st);
 
 constexpr int kStatsPad = 512;          // zero cells after the last t0 cell of every stats row
 constexpr size_t kAlign = 256;          // workspace carve-up alignment
+constexpr int kMaxClasses = 256;        // residue classes of a rational off-grid t0 stride (Geometry::cls)
+constexpr int kMaxClassStride = 64;     // ... and the samples between neighbouring cells of one class
 
 inline size_t align_up(size_t x, size_t a = kAlign) { return (x + a - 1) / a * a; }
 inline int64_t round_up64(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
@@ -52,7 +54,13 @@ struct Geometry {
     double cadence = 0.0;   // c, days
     bool on_grid = true;    // t0 grid sits on the sample grid with a whole-sample stride (R3), else R25
     int64_t n0 = 0;         // on_grid: sample index of t0 cell 0 (may be negative)
-    int64_t q = 0;          // on_grid: t0 stride in samples (>= 1)
+    int64_t q = 0;          // on_grid: t0 stride in samples (>= 1); rational: numerator p of stride / cadence = p / cls
+    // Off the sample grid, but stride / cadence = p / cls to within 1e-6 samples at the last cell (the paper's default
+    // stride on 2-min data is 18 s / 120 s = 3 / 20): the cells of one residue class i = cls a + rho then sit p whole
+    // samples apart at one common sub-sample offset, and each class is an on-grid problem with its own tap tables.
+    bool rational = false;
+    int64_t cls = 1;        // number of residue classes (1 on the sample grid)
+    double drift = 0.0;     // rational: bound on |i stride / cadence - i p / cls| over the grid, in samples
     double delta = 0.0;     // t0_start - times[0], days
     double stride = 0.0;    // t0 stride, days
 };

@@ -77,6 +77,89 @@ __global__ void build_taps_kernel(const __grid_constant__ LinearParams P, const 
     }
 }
 
+// Exact (R25) evaluations done by the fast off-grid paths since the last reset: cetra_exact_eval_count.
+__device__ unsigned long long g_exact_evals;
+
+int exact_eval_count(int64_t *count, bool reset) {
+    unsigned long long v = 0;
+    CETRA_CUDA_TRY(cudaMemcpyFromSymbol(&v, g_exact_evals, sizeof(v)));
+    if (count) *count = static_cast<int64_t>(v);
+    if (reset) {
+        v = 0;
+        CETRA_CUDA_TRY(cudaMemcpyToSymbol(g_exact_evals, &v, sizeof(v)));
+    }
+    return CETRA_OK;
+}
+
+// R25, one (sample, cell) pair exactly as the definition reads: every FP64 step one rounded IEEE operation.
+// Returns the template index, or -1 when the sample lies outside the window 0 <= x <= 1 (R2).
+__device__ __forceinline__ int r25_index(long long n, double ti, double c, double D, double Mm1) {
+    const double x = __dadd_rn(__ddiv_rn(__dsub_rn(__dmul_rn(static_cast<double>(n), c), ti), D), 0.5);
+    if (!(x >= 0.0 && x <= 1.0)) return -1;
+    return static_cast<int>(floor(__dadd_rn(__dmul_rn(x, Mm1), 0.5)));
+}
+
+// L1 for the residue classes of a rational off-grid stride.  Tap (b, a) of class rho is the sample k = q a + b - H_j
+// samples after the class's anchor sample; the cell sits f_rho samples after the anchor, so the tap's position in
+// the template is pos = ((k - f_rho) c / D + 1/2)(M - 1) + 1/2 for EVERY cell of the class, up to (i) the rounding
+// of the definition's own FP64 sequence (R25), which depends on the cell, and (ii) the drift of the stride from
+// p / cls.  Both are bounded by eps = eps_scale / D + eps_abs (see build_linear_plan).  A tap whose position is
+// further than eps from every decision point (an integer, where floor() steps, or a window edge) gets the same
+// template sample for every cell and goes into the table; the others are withheld (table entry 0, flag set) and
+// linear_search_kernel evaluates them per cell with r25_index.
+__global__ void build_class_taps_kernel(const __grid_constant__ LinearParams P, const double *__restrict__ cls_f,
+                                        double eps_scale, double eps_abs, float2 *__restrict__ taps,
+                                        unsigned char *__restrict__ flags) {
+    const int j = blockIdx.y, rho = blockIdx.z;
+    const int A = P.A[j], H = P.H[j], q = P.q;
+    const int stored = P.tap_off[j + 1] - P.tap_off[j];
+    const double D = P.durations[j], Mm1 = static_cast<double>(P.n_tpl - 1);
+    const double eps = eps_scale / D + eps_abs;
+    const double f = cls_f[rho];
+    const long long base = static_cast<long long>(P.n_cls) * P.tap_off[j] + static_cast<long long>(rho) * stored;
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < stored; idx += gridDim.x * blockDim.x) {
+        float m = 0.f;
+        unsigned char flag = 0;
+        if (idx < q * A) {
+            const int b = idx / A, a = idx - b * A;
+            const int kk = q * a + b;
+            if (kk <= 2 * H) {
+                const double u = static_cast<double>(kk - H) - f;
+                const double pos = (u * P.cadence / D + 0.5) * Mm1 + 0.5;
+                const bool near_step = fabs(pos - rint(pos)) < eps;
+                const bool near_edge = fabs(pos - 0.5) < eps || fabs(pos - (Mm1 + 0.5)) < eps;
+                if (near_step || near_edge) {
+                    flag = (pos > 0.5 - 2.0 * eps && pos < Mm1 + 0.5 + 2.0 * eps) ? 1 : 0;   // far outside: plainly 0
+                } else if (pos > 0.5 && pos < Mm1 + 0.5) {
+                    m = P.tpl[static_cast<int>(floor(pos))];
+                }
+            }
+        }
+        taps[base + idx] = make_float2(m, m * m);
+        flags[base + idx] = flag;
+    }
+}
+
+// One thread per (duration, class): the withheld taps of its table, as sample offsets k in table order.
+__global__ void collect_withheld_taps_kernel(const __grid_constant__ LinearParams P,
+                                             const unsigned char *__restrict__ flags, int *__restrict__ cnt,
+                                             int *__restrict__ list) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= P.n_dur * P.n_cls) return;
+    const int j = t / P.n_cls, rho = t - j * P.n_cls;
+    const int A = P.A[j], H = P.H[j], q = P.q;
+    const int stored = P.tap_off[j + 1] - P.tap_off[j];
+    const long long base = static_cast<long long>(P.n_cls) * P.tap_off[j] + static_cast<long long>(rho) * stored;
+    int n = 0;
+    for (int idx = 0; idx < q * A; ++idx) {
+        if (flags[base + idx]) {
+            const int b = idx / A, a = idx - b * A;
+            list[base + n++] = q * a + b - H;
+        }
+    }
+    cnt[t] = n;
+}
+
 // ------------------------------------------------------------------------------------------- L2 + L3
 // Packed FP32 (FFMA2 / FADD2 on sm_100a): both sufficient statistics of a cell in one issue slot.  The two
 // halves are independent IEEE fp32 operations with round-to-nearest, exactly fmaf / + on each component.
@@ -119,7 +202,13 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
     // grid = (tiles of a row, durations, light curves): consecutive blocks share a duration's tap table
     const long long lc = blockIdx.z;
     const int j = P.order[blockIdx.y];                          // longest durations first
-    const int tile = blockIdx.x;
+    int tile = blockIdx.x, rho = 0;                             // x = tile * n_cls + class: a tile's classes run together
+    if (P.n_cls > 1) {
+        tile = blockIdx.x / static_cast<unsigned int>(P.n_cls);
+        rho = blockIdx.x - tile * P.n_cls;
+    }
+    // cells of this class: i = n_cls a + rho < n_t0
+    const long long n_cells = P.n_cls > 1 ? (P.n_t0 - rho + P.n_cls - 1) / P.n_cls : P.n_t0;
     const int q = P.q;
     const int A = P.A[j];
     const long long i_blk = static_cast<long long>(tile) * TILE;
@@ -127,7 +216,8 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
     const int slice = (TILE + A + 2) & ~1;                       // samples of one branch (+ alignment slack)
 
     // element of the first tap of output 0 in the padded sample numbering; branch b starts b samples later
-    const unsigned int e0 = static_cast<unsigned int>(P.n0 - P.H[j] - P.n_lo);   // <= h_max + 2, far below 2^31
+    const long long n0c = P.n_cls > 1 ? static_cast<long long>(P.cls_n0[rho]) : P.n0;   // sample under (nearest to) cell 0
+    const unsigned int e0 = static_cast<unsigned int>(n0c - P.H[j] - P.n_lo);   // <= h_max + q + 4, far below 2^31
     const unsigned int uq = static_cast<unsigned int>(q);
 
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);      // bar[0], bar[1]: one per sample stage
@@ -146,7 +236,9 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
         if (b > 1) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the stage was read by generic loads
         mbar_arrive_expect_tx(bb, bytes + bytes_taps);
         bulk_copy_g2s_chunked(stage0 + (b & 1) * slice, P.wfw + (lc * q + v) * P.ph_pitch + (u0 - d0), bytes, bb);
-        if (with_taps) bulk_copy_g2s_chunked(taps, P.taps + P.tap_off[j], bytes_taps, bb);
+        if (with_taps)
+            bulk_copy_g2s_chunked(taps, P.taps + static_cast<long long>(P.n_cls) * P.tap_off[j] +
+                                            static_cast<long long>(rho) * n_tap, bytes_taps, bb);
     };
 
     if (tid == 0) {
@@ -156,14 +248,14 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
         issue(0, true);
     }
     __syncthreads();
-    if (P.stats && tile == P.tiles_per_row - 1) {               // zero the row padding (while the fill is in flight)
+    if (P.stats && tile == P.tiles_per_row - 1 && rho == 0) {   // zero the row padding (while the fill is in flight)
         const long long prow = lc * P.n_dur + j;
         for (long long i = P.n_t0 + tid; i < P.stats_pitch; i += WARPS * 32)
             P.stats[prow * P.stats_pitch + i] = make_float2(0.f, 0.f);
     }
     // a warp whose 32*R cells all lie past the last t0 cell has nothing to compute (last tile of a row); with
     // several polyphase branches every warp stays for the block-wide barriers between the branches
-    if (q == 1 && i_blk + static_cast<long long>(warp) * (32 * R) >= P.n_t0) return;
+    if (q == 1 && i_blk + static_cast<long long>(warp) * (32 * R) >= n_cells) return;
 
     // Two-level summation: the running FFMA accumulators are folded into a second set every kFlush tap
     // groups (and at the end of every polyphase branch), so that no FP32 sum runs over more than
@@ -213,6 +305,39 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
         }
         if (q > 1) __syncthreads();                              // every warp is done with this stage
     }
+    // The taps the class table withholds (positions within rounding of a decision point): evaluated per cell with
+    // the definition's own FP64 sequence.  Rare: a handful of taps in some classes, none in most.
+    if (P.n_cls > 1) {
+        const int cnt = P.unsafe_cnt[j * P.n_cls + rho];
+        if (cnt > 0) {
+            const int *lst = P.unsafe_k + static_cast<long long>(P.n_cls) * P.tap_off[j] + static_cast<long long>(rho) * n_tap;
+            const double D = P.durations[j], Mm1 = static_cast<double>(P.n_tpl - 1);
+            unsigned int done = 0;
+            for (int t = 0; t < cnt; ++t) {
+                const int k = lst[t];
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const long long a = i_blk + tid * R + r;
+                    const long long nn = n0c + a * q + k;
+                    if (a < n_cells && nn >= 0 && nn < P.n) {
+                        const long long i = a * P.n_cls + rho;
+                        const double ti = __dadd_rn(P.delta, __dmul_rn(static_cast<double>(i), P.stride));
+                        const int idx = r25_index(nn, ti, P.cadence, D, Mm1);
+                        ++done;
+                        if (idx >= 0) {
+                            const float m = __ldg(P.tpl + idx);
+                            const long long e = nn - P.n_lo;
+                            const long long u = e / q, v = e - u * q;
+                            const float2 sm = __ldg(P.wfw + (lc * q + v) * P.ph_pitch + u);
+                            tot[r].x = fmaf(m, sm.x, tot[r].x);          // S_wmf += m * (w f)
+                            tot[r].y = fmaf(m * m, sm.y, tot[r].y);      // S_wmm += m^2 * w
+                        }
+                    }
+                }
+            }
+            if (done && P.exact_evals) atomicAdd(P.exact_evals, static_cast<unsigned long long>(done));
+        }
+    }
     // transposition buffer of the epilogue: the consumed stages when there were several branches, else its own
     float2 *stage = q > 1 ? stage0 : stage0 + slice;
 
@@ -223,21 +348,23 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
     __syncwarp();
     const long long row = lc * P.n_dur + j;
     const long long i_warp = i_blk + static_cast<long long>(warp) * (32 * R);
-    const long long left_ll = P.n_t0 - i_warp - lane;           // cell r*32 + lane of the warp exists iff r*32 < left
+    const long long left_ll = n_cells - i_warp - lane;          // cell r*32 + lane of the warp exists iff r*32 < left
     const int left = left_ll > 32 * R ? 32 * R : static_cast<int>(left_ll);
     const float2 *sl = st + lane;
+    const long long i_first = (i_warp + lane) * P.n_cls + rho;  // t0 cell of the lane's first output; 32 n_cls apart
+    const int step = 32 * P.n_cls;
     if (P.stats) {                                               // the form the periodic search consumes: no division
-        float2 *out = P.stats + row * P.stats_pitch + i_warp + lane;
+        float2 *out = P.stats + row * P.stats_pitch + i_first;
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             if (r * 32 < left) {
                 const float2 ab = sl[r * 32];
-                out[r * 32] = ab.x > 0.f ? ab : make_float2(0.f, 0.f);   // no observation in the window: null
+                out[r * step] = ab.x > 0.f ? ab : make_float2(0.f, 0.f);   // no observation in the window: null
             }
         }
     }
     if (P.depth || P.var || P.dlogL) {
-        const long long o = row * P.n_t0 + i_warp + lane;
+        const long long o = row * P.n_t0 + i_first;
         const float nanv = __int_as_float(0x7fc00000);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
@@ -246,9 +373,9 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
                 const float a = ab.x, bsum = ab.y;
                 const bool null_cell = !(a > 0.f);              // no observation in the window
                 const float depth = null_cell ? nanv : bsum / a;
-                if (P.depth) P.depth[o + r * 32] = depth;
-                if (P.var) P.var[o + r * 32] = null_cell ? nanv : 1.0f / a;
-                if (P.dlogL) P.dlogL[o + r * 32] = null_cell ? nanv : 0.5f * bsum * depth;
+                if (P.depth) P.depth[o + r * step] = depth;
+                if (P.var) P.var[o + r * step] = null_cell ? nanv : 1.0f / a;
+                if (P.dlogL) P.dlogL[o + r * step] = null_cell ? nanv : 0.5f * bsum * depth;
             }
         }
     }
@@ -325,7 +452,8 @@ int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const d
     if (n_dur > CETRA_MAX_DURATIONS) return CETRA_ERR_UNSUPPORTED;
     int rc = derive_geometry(times_host, n, grid, &pl->geo);
     if (rc != CETRA_OK) return rc;
-    if (!pl->geo.on_grid) {
+    const bool classes = !pl->geo.on_grid && pl->geo.rational;
+    if (!pl->geo.on_grid && !classes) {
         // R25: per-cell evaluation; the (w f, w) row is the plain sample array, no tap tables
         if (n_lc > 65535) return CETRA_ERR_UNSUPPORTED;
         GeneralParams &G = pl->G;
@@ -349,6 +477,36 @@ int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const d
     P.n0 = pl->geo.n0;
     P.n_t0 = grid.n_t0;
     P.n_dur = n_dur;
+    P.n_cls = static_cast<int>(pl->geo.cls);
+    P.n_tpl = n_template;
+    P.n = n;
+    P.cadence = pl->geo.cadence; P.delta = pl->geo.delta; P.stride = pl->geo.stride;
+    long long n0_min = pl->geo.n0, n0_max = pl->geo.n0;
+    if (classes) {
+        // class rho: its cell 0 is t0 cell rho, at phi = (delta + rho stride) / c samples = anchor sample + f
+        pl->cls_n0.resize(P.n_cls);
+        pl->cls_f.resize(P.n_cls);
+        for (int rho = 0; rho < P.n_cls; ++rho) {
+            const double phi = (pl->geo.delta + static_cast<double>(rho) * pl->geo.stride) / pl->geo.cadence;
+            if (!(fabs(phi) < 1e9)) return CETRA_ERR_UNSUPPORTED;
+            const long long nn = llrint(phi);
+            pl->cls_n0[rho] = static_cast<int>(nn);
+            pl->cls_f[rho] = phi - static_cast<double>(nn);
+            if (rho == 0) n0_min = n0_max = nn;
+            n0_min = std::min(n0_min, nn);
+            n0_max = std::max(n0_max, nn);
+        }
+        // How far the position of a tap in the template, computed once per class, can lie from the position the
+        // definition's rounded FP64 sequence (R25) produces for one of the class's cells, in template samples:
+        // (6 T 2^-53 + drift c) (M - 1) / D for the time arithmetic (T: largest time magnitude, drift: Geometry),
+        // 32 M 2^-53 for the last two operations; doubled.
+        double t_max = std::max(fabs(pl->geo.delta), fabs(pl->geo.delta + static_cast<double>(grid.n_t0) * pl->geo.stride));
+        t_max = std::max(t_max, static_cast<double>(n) * pl->geo.cadence);
+        const double ulp = 1.1102230246251565e-16;
+        pl->eps_scale = 2.0 * (6.0 * t_max * ulp + pl->geo.drift * pl->geo.cadence) * static_cast<double>(n_template - 1);
+        pl->eps_abs = 2.0 * 32.0 * static_cast<double>(n_template) * ulp + 1e-12;
+    }
+    const long long cells_cls0 = (grid.n_t0 + P.n_cls - 1) / P.n_cls;     // class 0 has the most cells
     int h_max = 0, a_max = 0;
     P.tap_off[0] = 0;
     for (int j = 0; j < n_dur; ++j) {
@@ -357,7 +515,9 @@ int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const d
         // window half-reach in samples (R2): floor(D / 2c), one more where the taps' own rounded arithmetic
         // (build_taps_kernel) still places sample h + 1 inside 0 <= x <= 1
         double h = floor(D / (2.0 * pl->geo.cadence));
-        {
+        if (classes) {
+            h = floor(D / (2.0 * pl->geo.cadence) + 0.5) + 1.0;         // |k - f| c <= D / 2 with |f| <= 1/2, and one spare
+        } else {
             const volatile double kc = (h + 1.0) * pl->geo.cadence;
             const volatile double xr = kc / D;
             const volatile double x_hi = xr + 0.5, x_lo = -xr + 0.5;
@@ -375,7 +535,8 @@ int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const d
         h_max = std::max(h_max, P.H[j]);
         a_max = std::max(a_max, P.A[j]);
     }
-    pl->taps_total = P.tap_off[n_dur];
+    pl->taps_total = static_cast<long long>(P.tap_off[n_dur]) * P.n_cls;
+    if (pl->taps_total > 0x7fffffffLL) return CETRA_ERR_UNSUPPORTED;
     // durations by decreasing cost, so that the heavy blocks are scheduled first
     std::vector<int> ord(n_dur);
     for (int j = 0; j < n_dur; ++j) ord[j] = j;
@@ -387,8 +548,8 @@ int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const d
     int warps = 4;
     for (;;) {
         const int tile = warps * 32 * R;
-        const long long tiles = (grid.n_t0 + tile - 1) / tile;
-        const long long blocks = tiles * n_dur * n_lc;
+        const long long tiles = (cells_cls0 + tile - 1) / tile;
+        const long long blocks = tiles * n_dur * n_lc * P.n_cls;
         const bool fits = linear_smem_bytes(*pl, R, warps) <= static_cast<size_t>(smem_limit);
         if (warps == 1 || (fits && blocks >= 2LL * n_sm)) {
             if (!fits) return CETRA_ERR_UNSUPPORTED;
@@ -398,13 +559,14 @@ int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const d
     }
     pl->warps = warps;
     pl->tile = warps * 32 * R;
-    P.tiles_per_row = static_cast<int>((grid.n_t0 + pl->tile - 1) / pl->tile);
+    P.tiles_per_row = static_cast<int>((cells_cls0 + pl->tile - 1) / pl->tile);
     if (n_lc > 65535) return CETRA_ERR_UNSUPPORTED;          // light curves are the grid's z dimension
+    if (static_cast<long long>(P.tiles_per_row) * P.n_cls > 0x7fffffffLL) return CETRA_ERR_UNSUPPORTED;
     pl->smem_bytes = linear_smem_bytes(*pl, R, warps);
 
     // padded (w f, w) samples in q polyphase streams: element u of stream v is sample n_lo + q u + v
-    P.n_lo = P.n0 - h_max - 2;
-    const long long u_hi = (h_max + 2 + P.q) / P.q + static_cast<long long>(P.tiles_per_row) * pl->tile + a_max + 8;
+    P.n_lo = n0_min - h_max - 2;
+    const long long u_hi = (n0_max - n0_min + h_max + 2 + P.q) / P.q + static_cast<long long>(P.tiles_per_row) * pl->tile + a_max + 8;
     P.ph_pitch = round_up64(u_hi, 4);
     P.lc_pitch = P.ph_pitch * P.q;
     P.stats_pitch = cetra_stats_pitch(grid.n_t0);
@@ -416,6 +578,13 @@ size_t linear_workspace_bytes(const LinearPlan &pl, int32_t n_lc, int32_t n_temp
     b += align_up(sizeof(float2) * static_cast<size_t>(pl.P.lc_pitch) * n_lc);   // (w f, w)
     b += align_up(sizeof(float2) * static_cast<size_t>(pl.taps_total));          // taps
     b += align_up(sizeof(float) * static_cast<size_t>(n_template));              // template
+    if (pl.P.n_cls > 1) {                                                        // residue classes: see run_linear
+        b += align_up(sizeof(int) * static_cast<size_t>(pl.P.n_cls));
+        b += align_up(sizeof(double) * static_cast<size_t>(pl.P.n_cls));
+        b += align_up(sizeof(int) * static_cast<size_t>(pl.P.n_cls) * pl.P.n_dur);
+        b += align_up(sizeof(int) * static_cast<size_t>(pl.taps_total));
+        b += align_up(static_cast<size_t>(pl.taps_total));
+    }
     return b;
 }
 
@@ -423,7 +592,8 @@ template <int R, int WARPS>
 static int launch_linear(const LinearPlan &pl, const LinearParams &P, int32_t n_lc, cudaStream_t st) {
     auto k = linear_search_kernel<R, WARPS>;
     CETRA_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes));
-    const dim3 grid(static_cast<unsigned>(P.tiles_per_row), static_cast<unsigned>(P.n_dur), static_cast<unsigned>(n_lc));
+    const dim3 grid(static_cast<unsigned>(P.tiles_per_row) * static_cast<unsigned>(P.n_cls), static_cast<unsigned>(P.n_dur),
+                    static_cast<unsigned>(n_lc));
     k<<<grid, WARPS * 32, pl.smem_bytes, st>>>(P);
     CETRA_LAUNCH_CHECK();
     return CETRA_OK;
@@ -438,16 +608,50 @@ int run_linear(LinearPlan &pl, const void *flux_dev, const void *flux_err_dev, c
     Carver ws(workspace_dev);
     float2 *taps = ws.take<float2>(static_cast<size_t>(pl.taps_total));
     float *tpl = ws.take<float>(static_cast<size_t>(n_template));
-    float2 *wfw = ws.take<float2>(static_cast<size_t>(pl.P.lc_pitch) * n_lc);
+    unsigned long long *exact_evals = nullptr;                // diagnostics counter (a device variable of the library)
+    CETRA_CUDA_TRY(cudaGetSymbolAddress(reinterpret_cast<void **>(&exact_evals), g_exact_evals));
     LinearParams &P = pl.P;
+    const bool classes = pl.geo.on_grid ? false : pl.geo.rational;
+    int *cls_n0 = nullptr, *unsafe_cnt = nullptr, *unsafe_k = nullptr;
+    double *cls_f = nullptr;
+    unsigned char *flags = nullptr;
+    if (classes) {
+        cls_n0 = ws.take<int>(P.n_cls);
+        cls_f = ws.take<double>(P.n_cls);
+        unsafe_cnt = ws.take<int>(static_cast<size_t>(P.n_cls) * P.n_dur);
+        unsafe_k = ws.take<int>(static_cast<size_t>(pl.taps_total));
+        flags = ws.take<unsigned char>(static_cast<size_t>(pl.taps_total));
+    }
+    float2 *wfw = ws.take<float2>(static_cast<size_t>(pl.P.lc_pitch) * n_lc);
+    P.cls_n0 = cls_n0; P.unsafe_cnt = unsafe_cnt; P.unsafe_k = unsafe_k;
+    P.tpl = tpl;
+    P.exact_evals = exact_evals;
+    pl.G.exact_evals = exact_evals;
     P.wfw = wfw;
     P.taps = taps;
     P.depth = depth_dev; P.var = var_dev; P.dlogL = dlogL_dev;
     P.stats = reinterpret_cast<float2 *>(stats_dev);
 
-    if (!pl.geo.on_grid && !pl.taps_ready) {
+    if (!pl.geo.on_grid && !classes && !pl.taps_ready) {
         CETRA_CUDA_TRY(cudaMemcpyAsync(tpl, template_host, sizeof(float) * n_template,
                                        template_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+        pl.taps_ready = true;
+    }
+    if (classes && !pl.taps_ready) {
+        // the per-class anchors (small host arrays of the plan: copied before cudaMemcpyAsync returns), then the
+        // class tap tables and the lists of the taps they withhold
+        CETRA_CUDA_TRY(cudaMemcpyAsync(tpl, template_host, sizeof(float) * n_template,
+                                       template_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+        CETRA_CUDA_TRY(cudaMemcpyAsync(cls_n0, pl.cls_n0.data(), sizeof(int) * P.n_cls, cudaMemcpyHostToDevice, st));
+        CETRA_CUDA_TRY(cudaMemcpyAsync(cls_f, pl.cls_f.data(), sizeof(double) * P.n_cls, cudaMemcpyHostToDevice, st));
+        int max_stored = 0;
+        for (int j = 0; j < P.n_dur; ++j) max_stored = std::max(max_stored, P.tap_off[j + 1] - P.tap_off[j]);
+        dim3 g((max_stored + 255) / 256, P.n_dur, P.n_cls);
+        build_class_taps_kernel<<<g, 256, 0, st>>>(P, cls_f, pl.eps_scale, pl.eps_abs, taps, flags);
+        CETRA_LAUNCH_CHECK();
+        const int pairs = P.n_dur * P.n_cls;
+        collect_withheld_taps_kernel<<<(pairs + 63) / 64, 64, 0, st>>>(P, flags, unsafe_cnt, unsafe_k);
+        CETRA_LAUNCH_CHECK();
         pl.taps_ready = true;
     }
     if (!pl.taps_ready) {
@@ -466,7 +670,8 @@ int run_linear(LinearPlan &pl, const void *flux_dev, const void *flux_err_dev, c
     {
         const long long total = static_cast<long long>(n_lc) * P.lc_pitch;
         // off-grid plans keep the plain sample row (one stream)
-        const long long ph_q = pl.geo.on_grid ? P.q : 1, ph_pitch = pl.geo.on_grid ? P.ph_pitch : P.lc_pitch;
+        const bool streams = pl.geo.on_grid || classes;
+        const long long ph_q = streams ? P.q : 1, ph_pitch = streams ? P.ph_pitch : P.lc_pitch;
         const int blocks = static_cast<int>(std::min<long long>((total + 255) / 256, 148LL * 16));
         if (dtype == CETRA_F32)
             preprocess_kernel<float><<<blocks, 256, 0, st>>>(static_cast<const float *>(flux_dev),
@@ -478,7 +683,7 @@ int run_linear(LinearPlan &pl, const void *flux_dev, const void *flux_err_dev, c
                                                              ph_pitch, ph_q, P.n_lo);
         CETRA_LAUNCH_CHECK();
     }
-    if (!pl.geo.on_grid) {
+    if (!pl.geo.on_grid && !classes) {
         GeneralParams &G = pl.G;
         G.wfw = wfw; G.tpl = tpl;
         G.depth = depth_dev; G.var = var_dev; G.dlogL = dlogL_dev;

@@ -508,6 +508,32 @@ def test_linear_search_off_grid_t0(cfg, frac, torch_cuda, cetra, oracle_mod):
     assert np.allclose(a[~nul], 1.0 / o.depth_var[~nul], rtol=1e-5)
 
 
+def test_off_grid_default_stride_takes_the_exact_fallback(torch_cuda, cetra, oracle_mod):
+    """The paper's default t0 grid on 2-min data (stride 18 s = 3/20 of the cadence) starting ON a sample:
+    every 20th cell sits exactly on a sample, where the window centre lands exactly on a rounding boundary of the
+    nearest-neighbour index (x = 1/2 -> position 512.0 in a 1 024-sample template).  The class tap tables withhold
+    such taps and the kernel evaluates them per cell with the definition's FP64 sequence (R25): the
+    counter of exact evaluations must be > 0 and every cell must agree with the oracle."""
+    p = _problem(2)
+    stride = 0.01 * p.durations[0]
+    t0_start, n_t0 = p.times[0], 40000
+    o = oracle_mod.linear_search(p.times, p.flux, p.flux_err, p.durations, t0_start, stride, n_t0, p.template)
+    flux, err = _dev(torch_cuda, p.flux), _dev(torch_cuda, p.flux_err)
+    cetra.cetra_exact_eval_count(reset=True)
+    r = cetra.cetra_linear_search(p.times, flux, err, p.durations, t0_start, stride, n_t0, p.template)
+    n_exact = cetra.cetra_exact_eval_count()
+    worst = assert_linear_parity(r.depth.cpu().numpy(), r.depth_var.cpu().numpy(), r.dlogL.cpu().numpy(),
+                                 o.depth, o.depth_var, o.dlogL, what="config 2 default t0 grid")
+    print("default-grid worst", worst, "exact evaluations", n_exact)
+    assert n_exact > 0
+    # a stride that is not a small rational multiple of the cadence takes the per-cell kernel, same bar
+    stride2 = stride * (1.0 + 1.0 / 977.0)
+    o2 = oracle_mod.linear_search(p.times, p.flux, p.flux_err, p.durations, t0_start, stride2, 12000, p.template)
+    r2 = cetra.cetra_linear_search(p.times, flux, err, p.durations, t0_start, stride2, 12000, p.template)
+    assert_linear_parity(r2.depth.cpu().numpy(), r2.depth_var.cpu().numpy(), r2.dlogL.cpu().numpy(),
+                         o2.depth, o2.depth_var, o2.dlogL, what="config 2 irrational stride")
+
+
 def test_whole_path_off_grid_t0(torch_cuda, cetra, oracle_mod):
     """Linear + periodic search on the paper's default t0 grid through the batched entry point."""
     p = _problem(1)
