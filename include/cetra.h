@@ -128,9 +128,16 @@ int64_t cetra_stats_pitch(int64_t n_t0);
 /* ------------------------------------------------------------------------------------------
  * Periodic search (§2.3).
  *
- *  depth_dev, var_dev, dlogL_dev  [n_lc][n_dur][n_t0] float32: the linear-search grids.  (dlogL is
- *        accepted for symmetry with the paper's interface; Eq. 4 summed at the common depth depends
- *        on it only through 1/2 depth^2/var.)
+ *  depth_dev, var_dev  [n_lc][n_dur][n_t0] float32: the linear-search grids (NaN = null cell).
+ *  dlogL_dev      [n_lc][n_dur][n_t0] float32 or NULL: the per-transit likelihood ratios LR_e that Eq. 4 sums
+ *        (PAPER.md:137-143).  Eq. 4 summed at the common depth Z is
+ *            sum_e [LR_e - 1/2 (depth_e - Z)^2 / var_e] = sum_e (LR_e - 1/2 depth_e^2 / var_e) + 1/2 (sum B)^2 / sum A,
+ *        A = 1/var, B = depth/var.  For the linear search's own grids the first sum vanishes (LR_e = Eq. 2 =
+ *        1/2 depth_e^2 / var_e, P2) and the search runs on the two sufficient statistics; that is also
+ *        what NULL means.  When the grid passed here differs from 1/2 depth^2/var in some cell by more than 1e-5
+ *        of it (e.g. full log-likelihoods), the call searches with the literal three-term sum
+ *        instead (a plain, slower kernel; decided on the device, the call stays asynchronous), so the records
+ *        are Eq. 4's for whatever grid the caller supplies (R20).
  *  periods_host   [n_per] float64 days, each >= t0_stride
  *  dur_lo_host, dur_hi_host  optional [n_per] int32: half-open duration-index range searched for each
  *        period; NULL = every duration.  Durations with D_j >= P_k are always skipped

@@ -346,9 +346,10 @@ def cetra_periodic_search(depth, depth_var, dlogL, t0_start: float, t0_stride: f
     torch = _torch()
     lib = load_library()
     for t in (depth, depth_var, dlogL):
-        if not t.is_cuda or t.dtype != torch.float32:
+        if t is not None and (not t.is_cuda or t.dtype != torch.float32):
             raise TypeError("linear-search grids must be float32 CUDA tensors")
-    depth, depth_var, dlogL = depth.contiguous(), depth_var.contiguous(), dlogL.contiguous()
+    depth, depth_var = depth.contiguous(), depth_var.contiguous()
+    dlogL = dlogL.contiguous() if dlogL is not None else None      # None: LR_e = 1/2 depth^2/var (cetra.h)
     if depth.dim() == 2:
         n_lc, (n_dur, n_t0) = 1, depth.shape
     else:
@@ -362,7 +363,8 @@ def cetra_periodic_search(depth, depth_var, dlogL, t0_start: float, t0_stride: f
     ws = _workspace(torch, nbytes, depth.device, workspace)
     peaks = _peaks_tensor(torch, n_lc, n_per, depth.device)
     with torch.cuda.device(depth.device):
-        rc = lib.cetra_periodic_search(depth.data_ptr(), depth_var.data_ptr(), dlogL.data_ptr(), n_lc, n_dur, grid,
+        rc = lib.cetra_periodic_search(depth.data_ptr(), depth_var.data_ptr(),
+                                       dlogL.data_ptr() if dlogL is not None else None, n_lc, n_dur, grid,
                                        _dp(durations), _dp(periods), n_per, lo, hi, peaks.data_ptr(), ws.data_ptr(),
                                        ws.numel(), _stream_ptr(torch, stream))
     _check(rc, "cetra_periodic_search")

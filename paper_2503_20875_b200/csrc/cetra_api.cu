@@ -237,7 +237,9 @@ int cetra_exact_eval_count(int64_t *count, int32_t reset) {
 // ---------------------------------------------------------------------------------------- periodic
 size_t cetra_periodic_workspace_bytes(int32_t n_lc, int32_t n_dur, cetra_t0_grid grid, int32_t n_per) {
     if (n_lc < 1 || n_dur < 1 || n_per < 1 || grid.n_t0 < 1) return 0;
-    return periodic_workspace_bytes(n_lc, n_per) + stats_bytes(n_lc, n_dur, grid.n_t0);
+    // keys and period arrays, the (S_wmm, S_wmf) rows, and for a caller's likelihood-ratio grid its residual rows + flag
+    return periodic_workspace_bytes(n_lc, n_per) + stats_bytes(n_lc, n_dur, grid.n_t0) +
+           align_up(stats_bytes(n_lc, n_dur, grid.n_t0) / 2) + kAlign;
 }
 
 int cetra_periodic_search_stats(const float *stats_dev, int32_t n_lc, int32_t n_dur, cetra_t0_grid grid,
@@ -264,7 +266,6 @@ int cetra_periodic_search(const float *depth_dev, const float *var_dev, const fl
                           const double *periods_host, int32_t n_per, const int32_t *dur_lo_host,
                           const int32_t *dur_hi_host, cetra_peak *peaks_dev, void *workspace_dev,
                           size_t workspace_bytes, void *cuda_stream) {
-    (void)dlogL_dev;   // Eq. 4 summed at the common depth needs only depth and var (P4)
     if (!depth_dev || !var_dev || !peaks_dev || ((dur_lo_host == nullptr) != (dur_hi_host == nullptr)))
         return CETRA_ERR_INVALID_ARG;
     const Device d = device_or_default();   // argument errors are reported even where no device is visible
@@ -279,9 +280,13 @@ int cetra_periodic_search(const float *depth_dev, const float *var_dev, const fl
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     char *ws = static_cast<char *>(workspace_dev);
     float2 *stats = reinterpret_cast<float2 *>(ws + periodic_workspace_bytes(n_lc, n_per));
-    rc = run_grids_to_stats(depth_dev, var_dev, n_lc * n_dur, grid.n_t0, stats, st);
+    // dlogL given: Eq. 4 is summed with the caller's LR_e (R20); NULL: LR_e = 1/2 depth^2/var, the linear search's own
+    float *resid = reinterpret_cast<float *>(ws + periodic_workspace_bytes(n_lc, n_per) + stats_bytes(n_lc, n_dur, grid.n_t0));
+    int *literal = reinterpret_cast<int *>(reinterpret_cast<char *>(resid) + align_up(stats_bytes(n_lc, n_dur, grid.n_t0) / 2));
+    rc = run_grids_to_stats(depth_dev, var_dev, dlogL_dev, n_lc * n_dur, grid.n_t0, stats, resid, literal, st);
     if (rc != CETRA_OK) return rc;
-    return run_periodic(pl, stats, periods_host, dur_lo_host, dur_hi_host, true, peaks_dev, workspace_dev, st);
+    return run_periodic(pl, stats, periods_host, dur_lo_host, dur_hi_host, true, peaks_dev, workspace_dev, st,
+                        dlogL_dev ? resid : nullptr, dlogL_dev ? literal : nullptr);
 }
 
 // ----------------------------------------------------------------------------------------- batched

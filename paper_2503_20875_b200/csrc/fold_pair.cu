@@ -231,6 +231,7 @@ __global__ void __launch_bounds__(kGrpThreads, 1) fold_pair_argmax_kernel(const 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t ew = smem_u32(smem_raw + 16 + warp * 512);          // the warp's epoch words: 2 blocks x 32 x 8 B
 
+    if (P.literal && *P.literal) return;       // a caller's likelihood-ratio grid: fold_literal_argmax_kernel searches
     if (tid == 0) {
         mbar_init(bar, 1);
         mbar_fence_init();

@@ -247,6 +247,7 @@ __global__ void __launch_bounds__(kStrThreads, 1) fold_stream_argmax_kernel(cons
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t stage_bytes = static_cast<uint32_t>(stage_cells) * 8u;
 
+    if (P.literal && *P.literal) return;       // a caller's likelihood-ratio grid: fold_literal_argmax_kernel searches
     if (tid == 0) {
         for (int s = 0; s < kStrStages; ++s) {
             mbar_init(&sm->full[s], 1);

@@ -38,7 +38,9 @@ __global__ void finalize_peaks_kernel(const __grid_constant__ PeriodicParams P, 
             const int p = static_cast<int>(id - static_cast<unsigned int>(j) * static_cast<unsigned int>(P.n_t0));
             const float2 *row = P.stats + (lc * P.n_dur + j) * P.stats_pitch;
             const double r = P.r_cells[k];
-            float sa = 0.f, sb = 0.f;
+            const bool literal = P.literal && *P.literal;
+            const float *res = literal ? P.resid + (lc * P.n_dur + j) * P.stats_pitch : nullptr;
+            float sa = 0.f, sb = 0.f, sc = 0.f;
             int ntr = 0;
             for (long long e = 0;; ++e) {
                 const long long cell = p + __double2ll_rn(__dmul_rn(static_cast<double>(e), r));
@@ -46,11 +48,12 @@ __global__ void finalize_peaks_kernel(const __grid_constant__ PeriodicParams P, 
                 const float2 ab = row[cell];
                 sa += ab.x;
                 sb += ab.y;
+                if (literal) sc += res[cell];
                 ntr += ab.x > 0.f ? 1 : 0;
             }
             out.depth = sb / sa;                                     // common depth Z
             out.depth_var = 1.0f / sa;
-            out.lr = 0.5f * sb * out.depth;
+            out.lr = 0.5f * sb * out.depth + sc;                     // Eq. 4 summed at Z (sc = 0 unless literal)
             out.t0 = static_cast<float>(P.t0_start + static_cast<double>(p) * P.t0_stride);
             out.i_t0 = p; out.j_dur = j; out.n_transits = ntr;
         }
@@ -59,23 +62,98 @@ __global__ void finalize_peaks_kernel(const __grid_constant__ PeriodicParams P, 
 }
 
 // (depth, var) grids -> (S_wmm, S_wmf) rows: S_wmm = 1/var, S_wmf = depth/var, null (NaN) cells -> 0.
-__global__ void grids_to_stats_kernel(const float *__restrict__ depth, const float *__restrict__ var, long long n_rows,
-                                      long long n_t0, long long pitch, float2 *__restrict__ stats) {
+// With a likelihood-ratio grid: resid = dlogL - 1/2 depth^2/var per cell (what Eq. 4 summed at Z keeps of LR_e beyond
+// the two statistics: sum_e [LR_e - 1/2 (D_e - Z)^2 / var_e] = sum_e resid_e + 1/2 (sum B)^2 / sum A), and the flag
+// is raised when some cell's resid exceeds the rounding of a linear-search grid (whose dlogL IS 1/2 depth^2/var).
+__global__ void grids_to_stats_kernel(const float *__restrict__ depth, const float *__restrict__ var,
+                                      const float *__restrict__ dlogL, long long n_rows, long long n_t0,
+                                      long long pitch, float2 *__restrict__ stats, float *__restrict__ resid,
+                                      int *__restrict__ literal) {
     const long long total = n_rows * pitch;
+    bool differs = false;
     for (long long idx = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; idx < total;
          idx += static_cast<long long>(gridDim.x) * blockDim.x) {
         const long long rowid = idx / pitch;
         const long long i = idx - rowid * pitch;
         float2 out = make_float2(0.f, 0.f);
+        float c = 0.f;
         if (i < n_t0) {
             const float d = depth[rowid * n_t0 + i], v = var[rowid * n_t0 + i];
             if (isfinite(d) && isfinite(v) && v > 0.f) {
                 const float a = 1.0f / v;
                 const float b = d / v;
-                if (isfinite(a) && isfinite(b)) out = make_float2(a, b);
+                if (isfinite(a) && isfinite(b)) {
+                    out = make_float2(a, b);
+                    if (dlogL) {
+                        const float l = dlogL[rowid * n_t0 + i];
+                        const float ident = 0.5f * d * b;
+                        c = l - ident;
+                        // beyond FP32 rounding of the identity (relative), and large enough to move a log-likelihood
+                        // at all (1e-7 absolute: sums of a few dozen epochs stay far below the 5e-6 that parity allows)
+                        if (!(fabsf(c) <= 1e-5f * fabsf(ident) + 1e-7f)) differs = true;   // also NaN / inf
+                        if (!isfinite(c)) c = 0.f;
+                    }
+                }
             }
         }
         stats[idx] = out;
+        if (resid) resid[idx] = c;
+    }
+    if (literal && __any_sync(0xffffffffu, differs) && (threadIdx.x & 31) == 0) atomicOr(literal, 1);
+}
+
+// Periodic search on a caller's likelihood-ratio grid (literal Eq. 3-4): three sums per (period,
+// duration, phase).  One warp per (light curve, period, duration), lanes over phases, rows read through L1/L2: a
+// plain kernel for a rare call (the searches the library chains itself run on the two-statistic kernels).
+__device__ __forceinline__ unsigned int order_bits(float x) {          // monotone map float -> uint (any sign)
+    const unsigned int b = __float_as_uint(x);
+    return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+
+__global__ void __launch_bounds__(256) fold_literal_argmax_kernel(const __grid_constant__ PeriodicParams P) {
+    if (!(P.literal && *P.literal)) return;
+    const int lane = threadIdx.x & 31;
+    const long long warp0 = (blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x) >> 5;
+    const long long n_warps = (static_cast<long long>(gridDim.x) * blockDim.x) >> 5;
+    const long long units = static_cast<long long>(P.n_lc) * P.n_dur * P.n_per;
+    for (long long u = warp0; u < units; u += n_warps) {
+        const int k = static_cast<int>(u % P.n_per);
+        const long long rowid = u / P.n_per;                             // lc * n_dur + j
+        const int j = static_cast<int>(rowid % P.n_dur);
+        const long long lc = rowid / P.n_dur;
+        if (!(P.durations[j] < P.periods[k])) continue;
+        if (P.dur_lo && (j < P.dur_lo[k] || j >= P.dur_hi[k])) continue;
+        const double r = P.r_cells[k];
+        const double rc = ceil(r);
+        const int n_phase = rc < static_cast<double>(P.n_t0) ? static_cast<int>(rc) : P.n_t0;   // R10
+        const float2 *row = P.stats + rowid * P.stats_pitch;
+        const float *res = P.resid + rowid * P.stats_pitch;
+        unsigned long long best = 0ull;
+        for (int p = lane; p < n_phase; p += 32) {
+            float sa = 0.f, sb = 0.f, sc = 0.f;
+            for (long long e = 0;; ++e) {
+                const long long cell = p + __double2ll_rn(__dmul_rn(static_cast<double>(e), r));   // R11
+                if (cell > P.n_t0 - 1) break;
+                const float2 ab = __ldg(row + cell);
+                sa += ab.x;
+                sb += ab.y;
+                sc += __ldg(res + cell);
+            }
+            if (sa >= 1.17549435e-38f) {
+                const float lr = 0.5f * sb * (sb / sa) + sc;
+                if (lr == lr) {
+                    const unsigned int id = static_cast<unsigned int>(j) * static_cast<unsigned int>(P.n_t0) + p;
+                    const unsigned long long key = (static_cast<unsigned long long>(order_bits(lr)) << 32) | (0xffffffffu - id);
+                    best = key > best ? key : best;                      // ties: the smaller cell id has the larger key
+                }
+            }
+        }
+#pragma unroll
+        for (int s = 16; s > 0; s >>= 1) {
+            const unsigned long long o = __shfl_xor_sync(0xffffffffu, best, s);
+            best = o > best ? o : best;
+        }
+        if (lane == 0 && best) atomicMax(P.keys + lc * P.n_per + k, best);
     }
 }
 
@@ -132,7 +210,7 @@ size_t periodic_workspace_bytes(int32_t n_lc, int32_t n_per) {
 
 int run_periodic(PeriodicPlan &pl, const float2 *stats_dev, const double *periods_host, const int32_t *dur_lo_host,
                  const int32_t *dur_hi_host, bool upload, cetra_peak *peaks_dev, void *workspace_dev,
-                 cudaStream_t st) {
+                 cudaStream_t st, const float *resid_dev, const int *literal_dev) {
     PeriodicParams &P = pl.P;
     Carver ws(workspace_dev);
     double *periods = ws.take<double>(P.n_per);
@@ -161,6 +239,8 @@ int run_periodic(PeriodicPlan &pl, const float2 *stats_dev, const double *period
     P.dur_hi = ranges ? hi : nullptr;
     P.keys = keys;
     P.counter = reinterpret_cast<unsigned int *>(keys + n_keys);
+    P.resid = resid_dev;
+    P.literal = literal_dev;
     CETRA_CUDA_TRY(cudaMemsetAsync(keys, 0, sizeof(unsigned long long) * (n_keys + 32), st));
     profile_mark(kProfFold, true, st);
     {
@@ -169,6 +249,10 @@ int run_periodic(PeriodicPlan &pl, const float2 *stats_dev, const double *period
     }
     profile_mark(kProfFold, false, st);
     CETRA_LAUNCH_CHECK();
+    if (resid_dev && literal_dev) {                           // returns at once unless the flag is raised
+        fold_literal_argmax_kernel<<<148 * 8, 256, 0, st>>>(P);
+        CETRA_LAUNCH_CHECK();
+    }
     {
         const long long total = static_cast<long long>(P.n_lc) * P.n_per;
         const int blocks = static_cast<int>(std::min<long long>((total + 255) / 256, 148LL * 8));
@@ -178,12 +262,14 @@ int run_periodic(PeriodicPlan &pl, const float2 *stats_dev, const double *period
     return CETRA_OK;
 }
 
-int run_grids_to_stats(const float *depth_dev, const float *var_dev, int32_t n_rows, int64_t n_t0,
-                       float2 *stats_dev, cudaStream_t st) {
+int run_grids_to_stats(const float *depth_dev, const float *var_dev, const float *dlogL_dev, int32_t n_rows,
+                       int64_t n_t0, float2 *stats_dev, float *resid_dev, int *literal_dev, cudaStream_t st) {
     const long long pitch = cetra_stats_pitch(n_t0);
     const long long total = static_cast<long long>(n_rows) * pitch;
     const int blocks = static_cast<int>(std::min<long long>((total + 255) / 256, 148LL * 16));
-    grids_to_stats_kernel<<<blocks, 256, 0, st>>>(depth_dev, var_dev, n_rows, n_t0, pitch, stats_dev);
+    if (literal_dev) CETRA_CUDA_TRY(cudaMemsetAsync(literal_dev, 0, sizeof(int), st));
+    grids_to_stats_kernel<<<blocks, 256, 0, st>>>(depth_dev, var_dev, dlogL_dev, n_rows, n_t0, pitch, stats_dev,
+                                                  dlogL_dev ? resid_dev : nullptr, dlogL_dev ? literal_dev : nullptr);
     CETRA_LAUNCH_CHECK();
     return CETRA_OK;
 }

@@ -27,6 +27,11 @@ struct PeriodicParams {
     const int *dur_lo, *dur_hi;      // [n_per] device or null
     unsigned long long *keys;        // [n_lc][n_per] packed (lr bits << 32 | ~cell id), 0 = no candidate
     unsigned int *counter;           // work-unit queue head
+    // cetra_periodic_search with a caller's likelihood-ratio grid (literal Eq. 4): resid = dlogL - 1/2 depth^2/var per
+    // cell, and a device flag that is non-zero when some cell's resid matters (then fold_literal_argmax_kernel does
+    // the search and the two-statistic kernels return at once).  Both null on the sufficient-statistics path.
+    const float *resid;              // [n_lc][n_dur][stats_pitch] or null
+    const int *literal;              // device flag or null
     long long stats_pitch;
     double t0_start, t0_stride;
     int n_lc, n_dur, n_t0, n_per;
@@ -49,10 +54,10 @@ size_t periodic_workspace_bytes(int32_t n_lc, int32_t n_per);   // periods, rang
 // periods / ranges are uploaded when `upload` is set (first chunk of a batched search), else re-used.
 int run_periodic(PeriodicPlan &pl, const float2 *stats_dev, const double *periods_host, const int32_t *dur_lo_host,
                  const int32_t *dur_hi_host, bool upload, cetra_peak *peaks_dev, void *workspace_dev,
-                 cudaStream_t st);
+                 cudaStream_t st, const float *resid_dev = nullptr, const int *literal_dev = nullptr);
 int launch_fold_stream(const PeriodicPlan &pl, cudaStream_t st);   // fold_stream.cu
 int launch_fold_pair(const PeriodicPlan &pl, cudaStream_t st);     // fold_pair.cu
-int run_grids_to_stats(const float *depth_dev, const float *var_dev, int32_t n_rows, int64_t n_t0,
-                       float2 *stats_dev, cudaStream_t st);
+int run_grids_to_stats(const float *depth_dev, const float *var_dev, const float *dlogL_dev, int32_t n_rows,
+                       int64_t n_t0, float2 *stats_dev, float *resid_dev, int *literal_dev, cudaStream_t st);
 
 }  // namespace cetra

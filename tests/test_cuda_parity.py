@@ -233,6 +233,41 @@ def test_periodic_search_sampled_periods(cfg, n_random, torch_cuda, cetra, oracl
         assert np.all(full["j_dur"] < p.durations.shape[0])
 
 
+@pytest.mark.parametrize("cfg,kind", [(1, "random"), (1, "constant"), (2, "random")])
+def test_periodic_search_honours_a_callers_likelihood_grid(cfg, kind, torch_cuda, cetra, oracle_mod):
+    """Eq. 4 sums the per-transit likelihood ratios LR_e the caller passes.  For the linear
+    search's own grid LR_e = 1/2 depth^2/var and two statistics suffice; a grid that differs (here: offset per
+    cell, as when full log-likelihoods are passed) must give the literal sum, as the oracle does
+    (R20): the winners change, and GPU and oracle still agree.  dlogL = None means the identity."""
+    p = _problem(cfg)
+    g32, _ = _oracle_periodic_inputs(oracle_mod, cfg)
+    d32, v32, l32 = g32
+    rng = np.random.default_rng(77 + cfg)
+    off = (rng.uniform(0.0, 2.0, size=l32.shape) if kind == "random" else np.full(l32.shape, 1.0)).astype(np.float32)
+    l_off = (l32 + off).astype(np.float32)
+    l_off[np.isnan(l32)] = np.nan
+    import oracle as oracle_pkg
+    g64 = oracle_pkg.LinearGrids(d32.astype(np.float64), v32.astype(np.float64), l_off.astype(np.float64))
+    sel = np.arange(p.periods.shape[0]) if cfg == 1 else period_subset(p.periods, [], 60, seed=5)
+    periods = p.periods[sel]
+    dev = [_dev(torch_cuda, a) for a in (d32, v32, l_off)]
+    pk = cetra.peaks_to_numpy(cetra.cetra_periodic_search(*dev, p.t0_start, p.t0_stride, p.durations, periods))[0]
+    orc = oracle_mod.periodic_search(g64, p.t0_start, p.t0_stride, p.durations, periods)
+
+    def cell(k, j, ph):
+        return oracle_mod.periodic_cell(g64, p.t0_stride, periods[k], j, ph)
+
+    res = assert_periodic_parity(pk, orc, cell, what=f"cfg{cfg} caller LR grid ({kind})")
+    print("caller LR grid:", cfg, kind, res)
+    # the two-statistic search (dlogL = None, or the identity grid) picks other cells on this input
+    plain = cetra.peaks_to_numpy(cetra.cetra_periodic_search(dev[0], dev[1], None, p.t0_start, p.t0_stride,
+                                                             p.durations, periods))[0]
+    ident = cetra.peaks_to_numpy(cetra.cetra_periodic_search(dev[0], dev[1], _dev(torch_cuda, l32), p.t0_start,
+                                                             p.t0_stride, p.durations, periods))[0]
+    assert np.array_equal(plain.view(np.uint8), ident.view(np.uint8))
+    assert (plain["i_t0"] != pk["i_t0"]).any() and np.all(pk["lr"] > plain["lr"])
+
+
 def test_periodic_search_duration_ranges_and_empty_periods(torch_cuda, cetra, oracle_mod):
     """Per-period duration ranges, periods shorter than every duration (no candidate -> NaN
     record, indices -1) and periods longer than the baseline (a single epoch)."""
