@@ -180,10 +180,18 @@ int cetra_search_batched(const double *times_host, const void *flux_dev, const v
                          cetra_peak *peaks_dev,
                          void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
 
-/* Same search for a sequence of transit templates ("it may be worth running CETRA across a sequence of values" of
- * the impact parameter): templates_host is [n_templates][n_template] float32, peaks_dev is
- * [n_templates][n_lc][n_per]; template t's records are exactly those of cetra_search_batched with that template.
- * The workspace is the one of cetra_search_batched (the templates are searched one after the other on the stream). */
+/* Same search for a set of transit templates in one pass ("it may be worth running CETRA across a sequence of
+ * values" of the impact parameter): templates_host is [n_templates][n_template] float32, peaks_dev is
+ * [n_templates][n_lc][n_per]; template t's records are bit for bit those of cetra_search_batched with that template.
+ * Per chunk of light curves the samples are preprocessed once, the tap tables of all templates are built in one
+ * launch, and ONE linear-search launch (grid y = template x duration) writes the statistics grids of every template
+ * from those samples; the fold then runs once per template.  The workspace holds one statistics grid per template:
+ * query it with cetra_search_batched_templates_workspace_bytes (n_templates x n_dur <= 65 535). */
+size_t cetra_search_batched_templates_workspace_bytes(const double *times_host, int64_t n, int32_t n_lc,
+                                                      int32_t lc_chunk, const double *durations_host, int32_t n_dur,
+                                                      cetra_t0_grid grid, int32_t n_template, int32_t n_templates,
+                                                      int32_t n_per);
+
 int cetra_search_batched_templates(const double *times_host, const void *flux_dev, const void *flux_err_dev,
                                    cetra_dtype dtype, int64_t n, int32_t n_lc, int32_t lc_chunk,
                                    const double *durations_host, int32_t n_dur, cetra_t0_grid grid,

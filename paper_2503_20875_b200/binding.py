@@ -31,6 +31,7 @@ EXPORTED_SYMBOLS = (
     "cetra_linear_workspace_bytes", "cetra_linear_search", "cetra_exact_eval_count",
     "cetra_periodic_workspace_bytes", "cetra_periodic_search", "cetra_periodic_search_stats",
     "cetra_search_batched_workspace_bytes", "cetra_search_batched", "cetra_search_batched_templates",
+    "cetra_search_batched_templates_workspace_bytes",
     "cetra_search_batched_host_workspace_bytes", "cetra_search_batched_host",
     "cetra_profile_enable", "cetra_profile_read", "cetra_peak_probe_workspace_bytes", "cetra_peak_probe",
     "cetra_median_cadence", "cetra_resample_grid", "cetra_resample_workspace_bytes", "cetra_resample",
@@ -110,6 +111,8 @@ def load_library() -> ctypes.CDLL:
     lib.cetra_search_batched.restype = ctypes.c_int
     lib.cetra_search_batched.argtypes = [dp, vp, vp, ctypes.c_int, i64, i32, i32, dp, i32, cetra_t0_grid, fp, i32,
                                          dp, i32, ip, ip, vp, vp, sz, vp]
+    lib.cetra_search_batched_templates_workspace_bytes.restype = sz
+    lib.cetra_search_batched_templates_workspace_bytes.argtypes = [dp, i64, i32, i32, dp, i32, cetra_t0_grid, i32, i32, i32]
     lib.cetra_search_batched_templates.restype = ctypes.c_int
     lib.cetra_search_batched_templates.argtypes = [dp, vp, vp, ctypes.c_int, i64, i32, i32, dp, i32, cetra_t0_grid, fp,
                                                    i32, i32, dp, i32, ip, ip, vp, vp, sz, vp]
@@ -452,8 +455,8 @@ def cetra_search_batched_templates(times, flux, flux_err, durations, t0_start: f
     hi_arr, hi = _opt_i32(dur_hi)
     grid = _grid(t0_start, t0_stride, n_t0)
     n_dur, n_per = durations.shape[0], periods.shape[0]
-    nbytes = int(lib.cetra_search_batched_workspace_bytes(_dp(times), n, n_lc, int(lc_chunk), _dp(durations), n_dur,
-                                                          grid, tpl.shape[1], n_per))
+    nbytes = int(lib.cetra_search_batched_templates_workspace_bytes(_dp(times), n, n_lc, int(lc_chunk), _dp(durations),
+                                                                    n_dur, grid, tpl.shape[1], tpl.shape[0], n_per))
     ws = _workspace(torch, nbytes, flux.device, workspace)
     peaks = torch.empty((tpl.shape[0], n_lc, n_per, 8), dtype=torch.int32, device=flux.device)
     with torch.cuda.device(flux.device):

@@ -301,8 +301,9 @@ struct BatchedLayout {
 // 512 MiB of workspace.  Larger chunks mean fewer, longer launches (the linear kernel's ramp and tail are
 // amortised: 43 % -> 50 % of the FP32 peak from 14 to 64 curves); the periodic search reads every row from
 // global memory only a handful of times per launch, so L2 residency of the grids does not matter.
-int32_t default_chunk(int32_t n_lc, int32_t n_dur, int64_t n_t0) {
-    const size_t per_lc = sizeof(float2) * static_cast<size_t>(n_dur) * static_cast<size_t>(cetra_stats_pitch(n_t0));
+int32_t default_chunk(int32_t n_lc, int32_t n_dur, int64_t n_t0, int32_t n_templates) {
+    const size_t per_lc = sizeof(float2) * static_cast<size_t>(n_dur) * static_cast<size_t>(cetra_stats_pitch(n_t0)) *
+                          static_cast<size_t>(n_templates);
     const size_t budget = 512ull << 20;
     const size_t c = std::max<size_t>(1, budget / std::max<size_t>(per_lc, 1));
     // (65 535: light curves are the z dimension of the linear kernels' grids)
@@ -311,27 +312,30 @@ int32_t default_chunk(int32_t n_lc, int32_t n_dur, int64_t n_t0) {
 
 int plan_batched(const double *times_host, int64_t n, int32_t n_lc, int32_t lc_chunk, const double *durations_host,
                  int32_t n_dur, cetra_t0_grid grid, int32_t n_template, int32_t n_per, const Device &d,
-                 LinearPlan *lin, BatchedLayout *lay) {
-    if (n_lc < 1 || lc_chunk < 0 || n_per < 1) return CETRA_ERR_INVALID_ARG;
+                 LinearPlan *lin, BatchedLayout *lay, int32_t n_templates = 1) {
+    if (n_lc < 1 || lc_chunk < 0 || n_per < 1 || n_templates < 1) return CETRA_ERR_INVALID_ARG;
     if (n_dur < 1 || grid.n_t0 < 1) return CETRA_ERR_INVALID_ARG;
-    const int32_t chunk = lc_chunk > 0 ? std::min(lc_chunk, n_lc) : default_chunk(n_lc, n_dur, grid.n_t0);
+    const int32_t chunk = lc_chunk > 0 ? std::min(lc_chunk, n_lc) : default_chunk(n_lc, n_dur, grid.n_t0, n_templates);
     const int rc = build_linear_plan(times_host, n, chunk, durations_host, n_dur, grid, n_template, d.smem_optin,
-                                     d.n_sm, lin);
+                                     d.n_sm, lin, n_templates);
     if (rc != CETRA_OK) return rc;
     lay->chunk = chunk;
     lay->linear_bytes = linear_workspace_bytes(*lin, chunk, n_template);
-    lay->stats_bytes = stats_bytes(chunk, n_dur, grid.n_t0);
+    lay->stats_bytes = stats_bytes(chunk, n_dur, grid.n_t0) * static_cast<size_t>(n_templates);   // one grid per template
     lay->periodic_bytes = periodic_workspace_bytes(chunk, n_per);
     lay->total = lay->linear_bytes + lay->stats_bytes + lay->periodic_bytes;
     return CETRA_OK;
 }
 
-// Linear search then periodic search for light curves [lc0, lc0 + m) of a chunked batch.
+// Linear search then periodic search for light curves [lc0, lc0 + m) of a chunked batch.  With a template set
+// (lin.n_templates = T > 1) the light curves are preprocessed once and ONE linear launch writes the
+// T statistics grids ([T][m][n_dur][pitch]); the fold then runs once per template (its work is per template by
+// nature).  peaks_dev: records of light curve lc0 for template 0; template t's are peaks_tpl_stride records further.
 int run_chunk(LinearPlan &lin, const BatchedLayout &lay, const Device &d, const void *flux_dev,
               const void *flux_err_dev, cetra_dtype dtype, int64_t n, int32_t m, bool first,
               const double *durations_host, int32_t n_dur, cetra_t0_grid grid, const float *template_host,
               int32_t n_template, const double *periods_host, int32_t n_per, const int32_t *dur_lo_host,
-              const int32_t *dur_hi_host, cetra_peak *peaks_dev, char *ws, cudaStream_t st) {
+              const int32_t *dur_hi_host, cetra_peak *peaks_dev, size_t peaks_tpl_stride, char *ws, cudaStream_t st) {
     float *stats = reinterpret_cast<float *>(ws + lay.linear_bytes);
     int rc = run_linear(lin, flux_dev, flux_err_dev, dtype, n, m, template_host, n_template, false, nullptr, nullptr,
                         nullptr, stats, ws, st);
@@ -339,8 +343,14 @@ int run_chunk(LinearPlan &lin, const BatchedLayout &lay, const Device &d, const 
     PeriodicPlan per;
     rc = build_periodic_plan(m, n_dur, grid, durations_host, periods_host, n_per, d.smem_optin, d.n_sm, &per);
     if (rc != CETRA_OK) return rc;
-    return run_periodic(per, reinterpret_cast<const float2 *>(stats), periods_host, dur_lo_host, dur_hi_host, first,
-                        peaks_dev, ws + lay.linear_bytes + lay.stats_bytes, st);
+    const size_t grid_elems = static_cast<size_t>(m) * n_dur * static_cast<size_t>(cetra_stats_pitch(grid.n_t0));
+    for (int t = 0; t < lin.n_templates; ++t) {
+        rc = run_periodic(per, reinterpret_cast<const float2 *>(stats) + t * grid_elems, periods_host, dur_lo_host,
+                          dur_hi_host, first && t == 0, peaks_dev + t * peaks_tpl_stride,
+                          ws + lay.linear_bytes + lay.stats_bytes, st);
+        if (rc != CETRA_OK) return rc;
+    }
+    return CETRA_OK;
 }
 
 }  // namespace
@@ -363,29 +373,22 @@ int cetra_search_batched(const double *times_host, const void *flux_dev, const v
                          const double *periods_host, int32_t n_per, const int32_t *dur_lo_host,
                          const int32_t *dur_hi_host, cetra_peak *peaks_dev, void *workspace_dev,
                          size_t workspace_bytes, void *cuda_stream) {
-    if (!flux_dev || !flux_err_dev || !template_host || !periods_host || !peaks_dev ||
-        (dtype != CETRA_F32 && dtype != CETRA_F64) || ((dur_lo_host == nullptr) != (dur_hi_host == nullptr)))
-        return CETRA_ERR_INVALID_ARG;
-    const Device d = device_or_default();   // argument errors are reported even where no device is visible
-    int rc;
+    return cetra_search_batched_templates(times_host, flux_dev, flux_err_dev, dtype, n, n_lc, lc_chunk, durations_host,
+                                          n_dur, grid, template_host, n_template, 1, periods_host, n_per, dur_lo_host,
+                                          dur_hi_host, peaks_dev, workspace_dev, workspace_bytes, cuda_stream);
+}
+
+size_t cetra_search_batched_templates_workspace_bytes(const double *times_host, int64_t n, int32_t n_lc,
+                                                      int32_t lc_chunk, const double *durations_host, int32_t n_dur,
+                                                      cetra_t0_grid grid, int32_t n_template, int32_t n_templates,
+                                                      int32_t n_per) {
+    const Device d = device_or_default();
     LinearPlan lin;
     BatchedLayout lay;
-    rc = plan_batched(times_host, n, n_lc, lc_chunk, durations_host, n_dur, grid, n_template, n_per, d, &lin, &lay);
-    if (rc != CETRA_OK) return rc;
-    if (!workspace_dev || !aligned(workspace_dev) || workspace_bytes < lay.total) return CETRA_ERR_WORKSPACE;
-    if ((rc = require_device()) != CETRA_OK) return rc;
-    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    const size_t esz = dtype_size(dtype);
-    for (int32_t lc0 = 0; lc0 < n_lc; lc0 += lay.chunk) {
-        const int32_t m = std::min(lay.chunk, n_lc - lc0);
-        const char *fl = static_cast<const char *>(flux_dev) + static_cast<size_t>(lc0) * n * esz;
-        const char *er = static_cast<const char *>(flux_err_dev) + static_cast<size_t>(lc0) * n * esz;
-        rc = run_chunk(lin, lay, d, fl, er, dtype, n, m, lc0 == 0, durations_host, n_dur, grid, template_host,
-                       n_template, periods_host, n_per, dur_lo_host, dur_hi_host,
-                       peaks_dev + static_cast<size_t>(lc0) * n_per, static_cast<char *>(workspace_dev), st);
-        if (rc != CETRA_OK) return rc;
-    }
-    return CETRA_OK;
+    if (plan_batched(times_host, n, n_lc, lc_chunk, durations_host, n_dur, grid, n_template, n_per, d, &lin, &lay,
+                     n_templates) != CETRA_OK)
+        return 0;
+    return lay.total;
 }
 
 int cetra_search_batched_templates(const double *times_host, const void *flux_dev, const void *flux_err_dev,
@@ -395,15 +398,28 @@ int cetra_search_batched_templates(const double *times_host, const void *flux_de
                                    const double *periods_host, int32_t n_per, const int32_t *dur_lo_host,
                                    const int32_t *dur_hi_host, cetra_peak *peaks_dev, void *workspace_dev,
                                    size_t workspace_bytes, void *cuda_stream) {
-    if (!templates_host || !peaks_dev || n_templates < 1 || n_template < 2 || n_lc < 1 || n_per < 1)
+    if (!flux_dev || !flux_err_dev || !templates_host || !periods_host || !peaks_dev || n_templates < 1 ||
+        (dtype != CETRA_F32 && dtype != CETRA_F64) || ((dur_lo_host == nullptr) != (dur_hi_host == nullptr)))
         return CETRA_ERR_INVALID_ARG;
-    for (int32_t t = 0; t < n_templates; ++t) {               // one search per template
-        const int rc = cetra_search_batched(times_host, flux_dev, flux_err_dev, dtype, n, n_lc, lc_chunk,
-                                            durations_host, n_dur, grid,
-                                            templates_host + static_cast<size_t>(t) * n_template, n_template,
-                                            periods_host, n_per, dur_lo_host, dur_hi_host,
-                                            peaks_dev + static_cast<size_t>(t) * n_lc * n_per, workspace_dev,
-                                            workspace_bytes, cuda_stream);
+    const Device d = device_or_default();   // argument errors are reported even where no device is visible
+    int rc;
+    LinearPlan lin;
+    BatchedLayout lay;
+    rc = plan_batched(times_host, n, n_lc, lc_chunk, durations_host, n_dur, grid, n_template, n_per, d, &lin, &lay,
+                      n_templates);
+    if (rc != CETRA_OK) return rc;
+    if (!workspace_dev || !aligned(workspace_dev) || workspace_bytes < lay.total) return CETRA_ERR_WORKSPACE;
+    if ((rc = require_device()) != CETRA_OK) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const size_t esz = dtype_size(dtype);
+    for (int32_t lc0 = 0; lc0 < n_lc; lc0 += lay.chunk) {
+        const int32_t m = std::min(lay.chunk, n_lc - lc0);
+        const char *fl = static_cast<const char *>(flux_dev) + static_cast<size_t>(lc0) * n * esz;
+        const char *er = static_cast<const char *>(flux_err_dev) + static_cast<size_t>(lc0) * n * esz;
+        rc = run_chunk(lin, lay, d, fl, er, dtype, n, m, lc0 == 0, durations_host, n_dur, grid, templates_host,
+                       n_template, periods_host, n_per, dur_lo_host, dur_hi_host,
+                       peaks_dev + static_cast<size_t>(lc0) * n_per, static_cast<size_t>(n_lc) * n_per,
+                       static_cast<char *>(workspace_dev), st);
         if (rc != CETRA_OK) return rc;
     }
     return CETRA_OK;
@@ -458,7 +474,7 @@ int cetra_search_batched_host(const double *times_host, const void *flux_host, c
         CETRA_CUDA_TRY(cudaMemcpyAsync(fl_dev, fl, bytes, cudaMemcpyHostToDevice, st));
         CETRA_CUDA_TRY(cudaMemcpyAsync(er_dev, er, bytes, cudaMemcpyHostToDevice, st));
         rc = run_chunk(lin, lay, d, fl_dev, er_dev, dtype, n, m, lc0 == 0, durations_host, n_dur, grid,
-                       template_host, n_template, periods_host, n_per, dur_lo_host, dur_hi_host, pk_dev, ws, st);
+                       template_host, n_template, periods_host, n_per, dur_lo_host, dur_hi_host, pk_dev, 0, ws, st);
         if (rc != CETRA_OK) return rc;
         CETRA_CUDA_TRY(cudaMemcpyAsync(peaks_host + static_cast<size_t>(lc0) * n_per, pk_dev,
                                        sizeof(cetra_peak) * static_cast<size_t>(m) * n_per, cudaMemcpyDeviceToHost,

@@ -56,6 +56,8 @@ __global__ void preprocess_kernel(const T *__restrict__ flux, const T *__restric
 __global__ void build_taps_kernel(const __grid_constant__ LinearParams P, const float *__restrict__ tpl,
                                   int n_tpl, double cadence, float2 *__restrict__ taps) {
     const int j = blockIdx.y;
+    tpl += static_cast<long long>(blockIdx.z) * n_tpl;          // z: template of the set
+    taps += blockIdx.z * P.tset_taps;
     const int A = P.A[j], H = P.H[j], q = P.q;
     const int stored = P.tap_off[j + 1] - P.tap_off[j];
     const double D = P.durations[j];
@@ -110,8 +112,10 @@ __device__ __forceinline__ int r25_index(long long n, double ti, double c, doubl
 __global__ void build_class_taps_kernel(const __grid_constant__ LinearParams P, const double *__restrict__ cls_f,
                                         double eps_scale, double eps_abs, float2 *__restrict__ taps,
                                         unsigned char *__restrict__ flags) {
-    const int j = blockIdx.y, rho = blockIdx.z;
-    const int A = P.A[j], H = P.H[j], q = P.q;
+    const int j = blockIdx.y, tset = blockIdx.z / P.n_cls, rho = blockIdx.z - tset * P.n_cls;
+    const float *tpl = P.tpl + static_cast<long long>(tset) * P.n_tpl;
+    taps += tset * P.tset_taps;                                 // the flags depend on the geometry only: every template
+    const int A = P.A[j], H = P.H[j], q = P.q;                   // of the set writes the same ones
     const int stored = P.tap_off[j + 1] - P.tap_off[j];
     const double D = P.durations[j], Mm1 = static_cast<double>(P.n_tpl - 1);
     const double eps = eps_scale / D + eps_abs;
@@ -131,7 +135,7 @@ __global__ void build_class_taps_kernel(const __grid_constant__ LinearParams P, 
                 if (near_step || near_edge) {
                     flag = (pos > 0.5 - 2.0 * eps && pos < Mm1 + 0.5 + 2.0 * eps) ? 1 : 0;   // far outside: plainly 0
                 } else if (pos > 0.5 && pos < Mm1 + 0.5) {
-                    m = P.tpl[static_cast<int>(floor(pos))];
+                    m = tpl[static_cast<int>(floor(pos))];
                 }
             }
         }
@@ -192,7 +196,9 @@ __device__ __forceinline__ float2 add2f(float2 a, float2 b) {
     return r;
 }
 
-template <int R, int WARPS>
+// CLS: the cells are split into residue classes (rational off-grid stride); false on the sample grid, where the
+// class decode and the exact fix-up are compiled out.
+template <int R, int WARPS, bool CLS>
 __global__ void __launch_bounds__(WARPS * 32)
 linear_search_kernel(const __grid_constant__ LinearParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -201,14 +207,20 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
 
     // grid = (tiles of a row, durations, light curves): consecutive blocks share a duration's tap table
     const long long lc = blockIdx.z;
-    const int j = P.order[blockIdx.y];                          // longest durations first
+    int yy = blockIdx.y, tset = 0;                              // y = template * n_dur + duration rank
+    if (P.n_tset > 1) {
+        tset = yy / P.n_dur;
+        yy -= tset * P.n_dur;
+    }
+    const int j = P.order[yy];                                  // longest durations first
     int tile = blockIdx.x, rho = 0;                             // x = tile * n_cls + class: a tile's classes run together
-    if (P.n_cls > 1) {
-        tile = blockIdx.x / static_cast<unsigned int>(P.n_cls);
-        rho = blockIdx.x - tile * P.n_cls;
+    const int n_cls = CLS ? P.n_cls : 1;
+    if (CLS) {
+        tile = blockIdx.x / static_cast<unsigned int>(n_cls);
+        rho = blockIdx.x - tile * n_cls;
     }
     // cells of this class: i = n_cls a + rho < n_t0
-    const long long n_cells = P.n_cls > 1 ? (P.n_t0 - rho + P.n_cls - 1) / P.n_cls : P.n_t0;
+    const long long n_cells = CLS ? (P.n_t0 - rho + n_cls - 1) / n_cls : P.n_t0;
     const int q = P.q;
     const int A = P.A[j];
     const long long i_blk = static_cast<long long>(tile) * TILE;
@@ -216,7 +228,7 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
     const int slice = (TILE + A + 2) & ~1;                       // samples of one branch (+ alignment slack)
 
     // element of the first tap of output 0 in the padded sample numbering; branch b starts b samples later
-    const long long n0c = P.n_cls > 1 ? static_cast<long long>(P.cls_n0[rho]) : P.n0;   // sample under (nearest to) cell 0
+    const long long n0c = CLS ? static_cast<long long>(P.cls_n0[rho]) : P.n0;   // sample under (nearest to) cell 0
     const unsigned int e0 = static_cast<unsigned int>(n0c - P.H[j] - P.n_lo);   // <= h_max + q + 4, far below 2^31
     const unsigned int uq = static_cast<unsigned int>(q);
 
@@ -237,7 +249,7 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
         mbar_arrive_expect_tx(bb, bytes + bytes_taps);
         bulk_copy_g2s_chunked(stage0 + (b & 1) * slice, P.wfw + (lc * q + v) * P.ph_pitch + (u0 - d0), bytes, bb);
         if (with_taps)
-            bulk_copy_g2s_chunked(taps, P.taps + static_cast<long long>(P.n_cls) * P.tap_off[j] +
+            bulk_copy_g2s_chunked(taps, P.taps + tset * P.tset_taps + static_cast<long long>(n_cls) * P.tap_off[j] +
                                             static_cast<long long>(rho) * n_tap, bytes_taps, bb);
     };
 
@@ -249,7 +261,7 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
     }
     __syncthreads();
     if (P.stats && tile == P.tiles_per_row - 1 && rho == 0) {   // zero the row padding (while the fill is in flight)
-        const long long prow = lc * P.n_dur + j;
+        const long long prow = (static_cast<long long>(tset) * gridDim.z + lc) * P.n_dur + j;
         for (long long i = P.n_t0 + tid; i < P.stats_pitch; i += WARPS * 32)
             P.stats[prow * P.stats_pitch + i] = make_float2(0.f, 0.f);
     }
@@ -307,10 +319,10 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
     }
     // The taps the class table withholds (positions within rounding of a decision point): evaluated per cell with
     // the definition's own FP64 sequence.  Rare: a handful of taps in some classes, none in most.
-    if (P.n_cls > 1) {
-        const int cnt = P.unsafe_cnt[j * P.n_cls + rho];
+    if (CLS) {
+        const int cnt = P.unsafe_cnt[j * n_cls + rho];
         if (cnt > 0) {
-            const int *lst = P.unsafe_k + static_cast<long long>(P.n_cls) * P.tap_off[j] + static_cast<long long>(rho) * n_tap;
+            const int *lst = P.unsafe_k + static_cast<long long>(n_cls) * P.tap_off[j] + static_cast<long long>(rho) * n_tap;
             const double D = P.durations[j], Mm1 = static_cast<double>(P.n_tpl - 1);
             unsigned int done = 0;
             for (int t = 0; t < cnt; ++t) {
@@ -320,12 +332,12 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
                     const long long a = i_blk + tid * R + r;
                     const long long nn = n0c + a * q + k;
                     if (a < n_cells && nn >= 0 && nn < P.n) {
-                        const long long i = a * P.n_cls + rho;
+                        const long long i = a * n_cls + rho;
                         const double ti = __dadd_rn(P.delta, __dmul_rn(static_cast<double>(i), P.stride));
                         const int idx = r25_index(nn, ti, P.cadence, D, Mm1);
                         ++done;
                         if (idx >= 0) {
-                            const float m = __ldg(P.tpl + idx);
+                            const float m = __ldg(P.tpl + static_cast<long long>(tset) * P.n_tpl + idx);
                             const long long e = nn - P.n_lo;
                             const long long u = e / q, v = e - u * q;
                             const float2 sm = __ldg(P.wfw + (lc * q + v) * P.ph_pitch + u);
@@ -346,13 +358,13 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
 #pragma unroll
     for (int r = 0; r < R; ++r) st[lane * R + r] = make_float2(tot[r].y, tot[r].x);   // stored as (S_wmm, S_wmf)
     __syncwarp();
-    const long long row = lc * P.n_dur + j;
+    const long long row = (static_cast<long long>(tset) * gridDim.z + lc) * P.n_dur + j;
     const long long i_warp = i_blk + static_cast<long long>(warp) * (32 * R);
     const long long left_ll = n_cells - i_warp - lane;          // cell r*32 + lane of the warp exists iff r*32 < left
     const int left = left_ll > 32 * R ? 32 * R : static_cast<int>(left_ll);
     const float2 *sl = st + lane;
-    const long long i_first = (i_warp + lane) * P.n_cls + rho;  // t0 cell of the lane's first output; 32 n_cls apart
-    const int step = 32 * P.n_cls;
+    const long long i_first = (i_warp + lane) * n_cls + rho;    // t0 cell of the lane's first output; 32 n_cls apart
+    const int step = 32 * n_cls;
     if (P.stats) {                                               // the form the periodic search consumes: no division
         float2 *out = P.stats + row * P.stats_pitch + i_first;
 #pragma unroll
@@ -391,7 +403,7 @@ __global__ void __launch_bounds__(128) linear_general_kernel(const __grid_consta
     const long long i = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x;
     const int j = blockIdx.y;
     const long long lc = blockIdx.z;
-    const long long row = lc * P.n_dur + j;
+    const long long row = P.row0 + lc * P.n_dur + j;
     if (i >= P.n_t0) {
         if (P.stats && i < P.stats_pitch) P.stats[row * P.stats_pitch + i] = make_float2(0.f, 0.f);   // row padding
         return;
@@ -446,9 +458,12 @@ static size_t linear_smem_bytes(const LinearPlan &pl, int R, int warps) {
 
 int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const double *durations_host,
                       int32_t n_dur, cetra_t0_grid grid, int32_t n_template, int smem_limit, int n_sm,
-                      LinearPlan *pl) {
-    if (!times_host || !durations_host || n < 2 || n_lc < 1 || n_dur < 1 || grid.n_t0 < 1 || n_template < 2)
+                      LinearPlan *pl, int32_t n_templates) {
+    if (!times_host || !durations_host || n < 2 || n_lc < 1 || n_dur < 1 || grid.n_t0 < 1 || n_template < 2 ||
+        n_templates < 1)
         return CETRA_ERR_INVALID_ARG;
+    if (static_cast<long long>(n_templates) * n_dur > 65535) return CETRA_ERR_UNSUPPORTED;   // grid y dimension
+    pl->n_templates = n_templates;
     if (n_dur > CETRA_MAX_DURATIONS) return CETRA_ERR_UNSUPPORTED;
     int rc = derive_geometry(times_host, n, grid, &pl->geo);
     if (rc != CETRA_OK) return rc;
@@ -536,7 +551,9 @@ int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const d
         a_max = std::max(a_max, P.A[j]);
     }
     pl->taps_total = static_cast<long long>(P.tap_off[n_dur]) * P.n_cls;
-    if (pl->taps_total > 0x7fffffffLL) return CETRA_ERR_UNSUPPORTED;
+    if (pl->taps_total * n_templates > 0x7fffffffLL) return CETRA_ERR_UNSUPPORTED;
+    P.n_tset = n_templates;
+    P.tset_taps = pl->taps_total;
     // durations by decreasing cost, so that the heavy blocks are scheduled first
     std::vector<int> ord(n_dur);
     for (int j = 0; j < n_dur; ++j) ord[j] = j;
@@ -549,7 +566,7 @@ int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const d
     for (;;) {
         const int tile = warps * 32 * R;
         const long long tiles = (cells_cls0 + tile - 1) / tile;
-        const long long blocks = tiles * n_dur * n_lc * P.n_cls;
+        const long long blocks = tiles * n_dur * n_lc * P.n_cls * n_templates;
         const bool fits = linear_smem_bytes(*pl, R, warps) <= static_cast<size_t>(smem_limit);
         if (warps == 1 || (fits && blocks >= 2LL * n_sm)) {
             if (!fits) return CETRA_ERR_UNSUPPORTED;
@@ -576,9 +593,9 @@ int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const d
 size_t linear_workspace_bytes(const LinearPlan &pl, int32_t n_lc, int32_t n_template) {
     size_t b = 0;
     b += align_up(sizeof(float2) * static_cast<size_t>(pl.P.lc_pitch) * n_lc);   // (w f, w)
-    b += align_up(sizeof(float2) * static_cast<size_t>(pl.taps_total));          // taps
-    b += align_up(sizeof(float) * static_cast<size_t>(n_template));              // template
-    if (pl.P.n_cls > 1) {                                                        // residue classes: see run_linear
+    b += align_up(sizeof(float2) * static_cast<size_t>(pl.taps_total) * pl.n_templates);   // taps
+    b += align_up(sizeof(float) * static_cast<size_t>(n_template) * pl.n_templates);       // template(s)
+    if (!pl.geo.on_grid && pl.geo.rational) {                                    // residue classes: see run_linear
         b += align_up(sizeof(int) * static_cast<size_t>(pl.P.n_cls));
         b += align_up(sizeof(double) * static_cast<size_t>(pl.P.n_cls));
         b += align_up(sizeof(int) * static_cast<size_t>(pl.P.n_cls) * pl.P.n_dur);
@@ -588,12 +605,12 @@ size_t linear_workspace_bytes(const LinearPlan &pl, int32_t n_lc, int32_t n_temp
     return b;
 }
 
-template <int R, int WARPS>
+template <int R, int WARPS, bool CLS>
 static int launch_linear(const LinearPlan &pl, const LinearParams &P, int32_t n_lc, cudaStream_t st) {
-    auto k = linear_search_kernel<R, WARPS>;
+    auto k = linear_search_kernel<R, WARPS, CLS>;
     CETRA_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes));
-    const dim3 grid(static_cast<unsigned>(P.tiles_per_row) * static_cast<unsigned>(P.n_cls), static_cast<unsigned>(P.n_dur),
-                    static_cast<unsigned>(n_lc));
+    const dim3 grid(static_cast<unsigned>(P.tiles_per_row) * static_cast<unsigned>(P.n_cls),
+                    static_cast<unsigned>(P.n_dur) * static_cast<unsigned>(P.n_tset), static_cast<unsigned>(n_lc));
     k<<<grid, WARPS * 32, pl.smem_bytes, st>>>(P);
     CETRA_LAUNCH_CHECK();
     return CETRA_OK;
@@ -606,8 +623,9 @@ int run_linear(LinearPlan &pl, const void *flux_dev, const void *flux_err_dev, c
     // the tap tables come first: their place must not depend on n_lc, because the batched search builds
     // them once and then runs ragged last chunks with fewer light curves in the same workspace
     Carver ws(workspace_dev);
-    float2 *taps = ws.take<float2>(static_cast<size_t>(pl.taps_total));
-    float *tpl = ws.take<float>(static_cast<size_t>(n_template));
+    const int T = pl.n_templates;                             // template_host holds T templates of n_template samples
+    float2 *taps = ws.take<float2>(static_cast<size_t>(pl.taps_total) * T);
+    float *tpl = ws.take<float>(static_cast<size_t>(n_template) * T);
     unsigned long long *exact_evals = nullptr;                // diagnostics counter (a device variable of the library)
     CETRA_CUDA_TRY(cudaGetSymbolAddress(reinterpret_cast<void **>(&exact_evals), g_exact_evals));
     LinearParams &P = pl.P;
@@ -633,20 +651,20 @@ int run_linear(LinearPlan &pl, const void *flux_dev, const void *flux_err_dev, c
     P.stats = reinterpret_cast<float2 *>(stats_dev);
 
     if (!pl.geo.on_grid && !classes && !pl.taps_ready) {
-        CETRA_CUDA_TRY(cudaMemcpyAsync(tpl, template_host, sizeof(float) * n_template,
+        CETRA_CUDA_TRY(cudaMemcpyAsync(tpl, template_host, sizeof(float) * n_template * T,
                                        template_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
         pl.taps_ready = true;
     }
     if (classes && !pl.taps_ready) {
         // the per-class anchors (small host arrays of the plan: copied before cudaMemcpyAsync returns), then the
         // class tap tables and the lists of the taps they withhold
-        CETRA_CUDA_TRY(cudaMemcpyAsync(tpl, template_host, sizeof(float) * n_template,
+        CETRA_CUDA_TRY(cudaMemcpyAsync(tpl, template_host, sizeof(float) * n_template * T,
                                        template_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
         CETRA_CUDA_TRY(cudaMemcpyAsync(cls_n0, pl.cls_n0.data(), sizeof(int) * P.n_cls, cudaMemcpyHostToDevice, st));
         CETRA_CUDA_TRY(cudaMemcpyAsync(cls_f, pl.cls_f.data(), sizeof(double) * P.n_cls, cudaMemcpyHostToDevice, st));
         int max_stored = 0;
         for (int j = 0; j < P.n_dur; ++j) max_stored = std::max(max_stored, P.tap_off[j + 1] - P.tap_off[j]);
-        dim3 g((max_stored + 255) / 256, P.n_dur, P.n_cls);
+        dim3 g((max_stored + 255) / 256, P.n_dur, P.n_cls * T);
         build_class_taps_kernel<<<g, 256, 0, st>>>(P, cls_f, pl.eps_scale, pl.eps_abs, taps, flags);
         CETRA_LAUNCH_CHECK();
         const int pairs = P.n_dur * P.n_cls;
@@ -655,14 +673,11 @@ int run_linear(LinearPlan &pl, const void *flux_dev, const void *flux_err_dev, c
         pl.taps_ready = true;
     }
     if (!pl.taps_ready) {
-        if (template_on_device) {
-            CETRA_CUDA_TRY(cudaMemcpyAsync(tpl, template_host, sizeof(float) * n_template, cudaMemcpyDeviceToDevice, st));
-        } else {
-            CETRA_CUDA_TRY(cudaMemcpyAsync(tpl, template_host, sizeof(float) * n_template, cudaMemcpyHostToDevice, st));
-        }
+        CETRA_CUDA_TRY(cudaMemcpyAsync(tpl, template_host, sizeof(float) * n_template * T,
+                                       template_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
         int max_stored = 0;
         for (int j = 0; j < P.n_dur; ++j) max_stored = std::max(max_stored, P.tap_off[j + 1] - P.tap_off[j]);
-        dim3 g((max_stored + 255) / 256, P.n_dur);
+        dim3 g((max_stored + 255) / 256, P.n_dur, T);
         build_taps_kernel<<<g, 256, 0, st>>>(P, tpl, n_template, pl.geo.cadence, taps);
         CETRA_LAUNCH_CHECK();
         pl.taps_ready = true;
@@ -685,25 +700,32 @@ int run_linear(LinearPlan &pl, const void *flux_dev, const void *flux_err_dev, c
     }
     if (!pl.geo.on_grid && !classes) {
         GeneralParams &G = pl.G;
-        G.wfw = wfw; G.tpl = tpl;
+        G.wfw = wfw;
         G.depth = depth_dev; G.var = var_dev; G.dlogL = dlogL_dev;
         G.stats = reinterpret_cast<float2 *>(stats_dev);
         const long long cells = stats_dev ? G.stats_pitch : G.n_t0;
         const dim3 g(static_cast<unsigned>((cells + 127) / 128), static_cast<unsigned>(G.n_dur),
                      static_cast<unsigned>(n_lc));
         profile_mark(kProfLinear, true, st);
-        linear_general_kernel<<<g, 128, 0, st>>>(G);
+        for (int t = 0; t < T; ++t) {                           // one launch per template of the set
+            G.tpl = tpl + static_cast<size_t>(t) * n_template;
+            G.row0 = static_cast<long long>(t) * n_lc * G.n_dur;
+            linear_general_kernel<<<g, 128, 0, st>>>(G);
+            CETRA_LAUNCH_CHECK();
+        }
         profile_mark(kProfLinear, false, st);
-        CETRA_LAUNCH_CHECK();
         return CETRA_OK;
     }
     constexpr int R = kLinearR;
     profile_mark(kProfLinear, true, st);
     int rc;
-    switch (pl.warps) {
-        case 4: rc = launch_linear<R, 4>(pl, P, n_lc, st); break;
-        case 2: rc = launch_linear<R, 2>(pl, P, n_lc, st); break;
-        default: rc = launch_linear<R, 1>(pl, P, n_lc, st); break;
+    switch (pl.warps * 2 + (classes ? 1 : 0)) {
+        case 8: rc = launch_linear<R, 4, false>(pl, P, n_lc, st); break;
+        case 9: rc = launch_linear<R, 4, true>(pl, P, n_lc, st); break;
+        case 4: rc = launch_linear<R, 2, false>(pl, P, n_lc, st); break;
+        case 5: rc = launch_linear<R, 2, true>(pl, P, n_lc, st); break;
+        case 2: rc = launch_linear<R, 1, false>(pl, P, n_lc, st); break;
+        default: rc = launch_linear<R, 1, true>(pl, P, n_lc, st); break;
     }
     profile_mark(kProfLinear, false, st);
     return rc;

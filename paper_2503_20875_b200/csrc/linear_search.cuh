@@ -20,6 +20,11 @@ struct LinearParams {
     // Residue classes of a rational off-grid stride (Geometry::rational): cell i = n_cls a + rho of class rho sits
     // q a samples after sample cls_n0[rho] + f_rho, |f_rho| <= 1/2.  n_cls = 1 on the sample grid (n0, no lists).
     int n_cls, n_tpl;
+    // Template set (cetra_search_batched_templates): T templates searched in one launch over the
+    // same preprocessed samples.  Template t has its own tap tables (tset_taps entries after those of t - 1), its
+    // own copy of the template (n_tpl floats after t - 1's) and its own output rows ((t n_lc + lc) n_dur + j).
+    int n_tset;
+    long long tset_taps;
     const int *cls_n0;          // [n_cls] device
     const int *unsafe_cnt;      // [n_dur][n_cls] device: taps of (j, rho) whose table entry is withheld (see build_class_taps_kernel)
     const int *unsafe_k;        // their sample offsets k, list of (j, rho) at n_cls * tap_off[j] + rho * stored_j
@@ -42,6 +47,7 @@ struct GeneralParams {
     float2 *stats;              // [n_lc][n_dur][stats_pitch] or null
     long long lc_pitch, n, n_t0, stats_pitch;
     int n_dur, n_tpl;
+    long long row0;                    // output row of (light curve 0, duration 0): template t of a set starts at t n_lc n_dur
     double cadence, delta, stride;
     unsigned long long *exact_evals;   // device counter of exact (R25) evaluations, diagnostics
     double eps_scale, eps_abs;         // a position closer than eps_scale / D + eps_abs to a decision point is evaluated exactly
@@ -59,11 +65,12 @@ struct LinearPlan {
     long long taps_total = 0;
     size_t smem_bytes = 0;
     bool taps_ready = false;    // tap tables already built in this workspace (batched path re-uses them)
+    int n_templates = 1;        // templates searched per launch (cetra_search_batched_templates)
 };
 
 int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const double *durations_host,
                       int32_t n_dur, cetra_t0_grid grid, int32_t n_template, int smem_limit, int n_sm,
-                      LinearPlan *pl);
+                      LinearPlan *pl, int32_t n_templates = 1);
 int exact_eval_count(int64_t *count, bool reset);
 size_t linear_workspace_bytes(const LinearPlan &pl, int32_t n_lc, int32_t n_template);
 int run_linear(LinearPlan &pl, const void *flux_dev, const void *flux_err_dev, cetra_dtype dtype, int64_t n,

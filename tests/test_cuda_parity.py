@@ -453,6 +453,17 @@ def test_template_sequence_equals_one_search_per_template(torch_cuda, cetra, ora
     orc = oracle_mod.periodic_search(o, p.t0_start, p.t0_stride, p.durations, p.periods)
     assert_periodic_parity(pk[2][1], orc, lambda k, j, ph: oracle_mod.periodic_cell(o, p.t0_stride, p.periods[k], j, ph),
                            what="template b = 0.99")
+    # chunks of two light curves (ragged last chunk), and the paper's default off-grid stride (one linear launch
+    # over the templates' class tap tables): still the records of one search per template
+    pk2 = cetra.peaks_to_numpy(cetra.cetra_search_batched_templates(p.times, flux, err, *args, tpls, p.periods,
+                                                                    lc_chunk=2).reshape(9, 300, 8)).reshape(3, 3, 300)
+    assert np.array_equal(pk2.view(np.uint8), pk.view(np.uint8))
+    og = (p.durations, p.times[0], 0.01 * p.durations[0], 30000)
+    pk3 = cetra.peaks_to_numpy(cetra.cetra_search_batched_templates(p.times, flux, err, *og, tpls, p.periods[:40],
+                                                                    lc_chunk=2).reshape(9, 40, 8)).reshape(3, 3, 40)
+    for t in range(3):
+        one = cetra.peaks_to_numpy(cetra.cetra_search_batched(p.times, flux, err, *og, tpls[t], p.periods[:40]))
+        assert np.array_equal(one.view(np.uint8), pk3[t].view(np.uint8))
 
 
 def test_bench_configuration_sampled_against_oracle(torch_cuda, cetra, oracle_mod):
@@ -567,6 +578,13 @@ def test_off_grid_default_stride_takes_the_exact_fallback(torch_cuda, cetra, ora
     r2 = cetra.cetra_linear_search(p.times, flux, err, p.durations, t0_start, stride2, 12000, p.template)
     assert_linear_parity(r2.depth.cpu().numpy(), r2.depth_var.cpu().numpy(), r2.dlogL.cpu().numpy(),
                          o2.depth, o2.depth_var, o2.dlogL, what="config 2 irrational stride")
+    # a whole-sample stride whose START is off the sample grid: a single residue class with a sub-sample offset
+    c = p.times[1] - p.times[0]
+    for start in (p.times[0] + 0.3 * c, p.times[0] - 100.5 * c):      # the second puts every cell half-way between samples
+        o3 = oracle_mod.linear_search(p.times, p.flux, p.flux_err, p.durations, start, 2 * c, 9000, p.template)
+        r3 = cetra.cetra_linear_search(p.times, flux, err, p.durations, start, 2 * c, 9000, p.template)
+        assert_linear_parity(r3.depth.cpu().numpy(), r3.depth_var.cpu().numpy(), r3.dlogL.cpu().numpy(),
+                             o3.depth, o3.depth_var, o3.dlogL, what="config 2 whole-sample stride, off-grid start")
 
 
 def test_whole_path_off_grid_t0(torch_cuda, cetra, oracle_mod):
