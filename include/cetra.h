@@ -73,7 +73,10 @@ typedef struct {
     float lr;           /* log-likelihood gain of the periodic model over the flat model (Eq. 4 summed) */
     float depth;        /* common depth Z */
     float depth_var;    /* its variance; SNR = depth / sqrt(depth_var) */
-    float t0;           /* t0_start + i_t0 * t0_stride, days */
+    float t0;           /* t0_start + i_t0 * t0_stride in days, ROUNDED TO FLOAT32: a convenience value.  i_t0 is the
+                         * result; with a large time origin (BJD - 2 457 000 ~ 3e3 d: float32 resolves 20 s; full BJD:
+                         * 0.25 d) recompute the time from i_t0 in double, or keep times relative to the first sample
+                         * as the paper does */
     int32_t i_t0;       /* cell of the first epoch, in [0, ceil(P/stride)) */
     int32_t j_dur;      /* duration index */
     int32_t n_transits; /* epochs that contributed (non-null cells) */
@@ -218,6 +221,13 @@ int cetra_search_batched_host(const double *times_host, const void *flux_host, c
                               const int32_t *dur_lo_host, const int32_t *dur_hi_host,
                               cetra_peak *peaks_host,
                               void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* Transit model -> search template ("The chosen/supplied model is ultimately resampled to a
+ * user-defined number of samples using simple linear interpolation").  model_host [n_model] float32 spans first to
+ * last contact; template_host [n_template] receives the model at n_template evenly spaced positions over the same
+ * span (both end samples kept), interpolated linearly in FP64 and rounded to float32.  A host-side setup helper
+ * (no device work).  Returns CETRA_OK or CETRA_ERR_INVALID_ARG (null pointer, fewer than 2 samples). */
+int cetra_resample_template(const float *model_host, int32_t n_model, float *template_host, int32_t n_template);
 
 /* ------------------------------------------------------------------------------------------
  * Setup: light-curve resampling (§2.1.1, lines 53-61).

@@ -51,6 +51,8 @@ def _load() -> ctypes.CDLL:
         lib.oracle_periodic_cell.argtypes = [dp, dp, dp, ctypes.c_int32, ctypes.c_int64, ctypes.c_double,
                                              ctypes.c_double, ctypes.c_int32, ctypes.c_int64,
                                              dp, dp, dp, ip]
+        lib.oracle_resample_template.restype = ctypes.c_int
+        lib.oracle_resample_template.argtypes = [dp, ctypes.c_int32, dp, ctypes.c_int32]
         lib.oracle_median_cadence.restype = ctypes.c_int
         lib.oracle_median_cadence.argtypes = [dp, ctypes.c_int64, dp]
         lib.oracle_resample.restype = ctypes.c_int
@@ -163,6 +165,17 @@ def periodic_cell(grids: LinearGrids, t0_stride: float, period: float, j: int, p
 
 
 # ------------------------------------------------------------------------- setup and follow-up steps
+def resample_template(model, n_out: int) -> np.ndarray:
+    """Supplied transit model -> n_out-sample template by linear interpolation."""
+    lib = _load()
+    model = _d(model)
+    out = np.empty(int(n_out))
+    rc = lib.oracle_resample_template(_p(model, ctypes.c_double), model.shape[0], _p(out, ctypes.c_double), int(n_out))
+    if rc != 0:
+        raise ValueError(f"oracle_resample_template failed with status {rc}")
+    return out
+
+
 def median_cadence(times) -> float:
     """Default resample cadence: the median cadence of the input (R22)."""
     lib = _load()

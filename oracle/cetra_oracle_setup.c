@@ -4,6 +4,7 @@
  * Plain FP64 restatements of the steps around the two searches (citations are
  * /root/reference/PAPER.md line numbers):
  *
+ *   oracle_resample_template  supplied transit model -> M-sample template by linear interpolation
  *   oracle_median_cadence   default resample cadence = median cadence of the input
  *   oracle_resample         irregular light curve -> regular grid: every observation goes to the
  *                           nearest output point; several observations in one point are combined
@@ -43,6 +44,20 @@
 static int cmp_double(const void *a, const void *b) {
     const double x = *(const double *)a, y = *(const double *)b;
     return (x > y) - (x < y);
+}
+
+/* "resampled to a user-defined number of samples using simple linear interpolation".
+ * Output sample m sits at fraction m/(n_out-1) of the model's span (first to last contact, both kept). */
+int oracle_resample_template(const double *model, int32_t n_in, double *out, int32_t n_out) {
+    if (n_in < 2 || n_out < 2) return ORACLE_ERR_ARG;
+    for (int32_t m = 0; m < n_out; ++m) {
+        const double pos = (double)m / (double)(n_out - 1) * (double)(n_in - 1);    /* in model samples */
+        int32_t lo = (int32_t)floor(pos);
+        if (lo >= n_in - 1) lo = n_in - 2;
+        const double w = pos - (double)lo;
+        out[m] = (1.0 - w) * model[lo] + w * model[lo + 1];
+    }
+    return ORACLE_OK;
 }
 
 /* R22 */

@@ -34,7 +34,7 @@ EXPORTED_SYMBOLS = (
     "cetra_search_batched_templates_workspace_bytes",
     "cetra_search_batched_host_workspace_bytes", "cetra_search_batched_host",
     "cetra_profile_enable", "cetra_profile_read", "cetra_peak_probe_workspace_bytes", "cetra_peak_probe",
-    "cetra_median_cadence", "cetra_resample_grid", "cetra_resample_workspace_bytes", "cetra_resample",
+    "cetra_resample_template", "cetra_median_cadence", "cetra_resample_grid", "cetra_resample_workspace_bytes", "cetra_resample",
     "cetra_monotransit_workspace_bytes", "cetra_monotransit_search",
     "cetra_mask_workspace_bytes", "cetra_mask_transits",
 )
@@ -187,6 +187,27 @@ def _torch():
     return torch
 
 
+def _on_stream(fn):
+    """Run a wrapper with `stream` as torch's current stream: the implicit workspace, the output tensors and any
+    `.contiguous()` copy of an input are then allocated and produced on the stream the kernels are enqueued on, and
+    the caching allocator ties their lifetime to that stream (a workspace freed on return is not handed to a tensor
+    of another stream while the kernels still use it).  Inputs produced on a different stream are the caller's to
+    order, as everywhere in torch."""
+    import functools
+    import inspect
+    sig = inspect.signature(fn)
+
+    @functools.wraps(fn)
+    def wrapper(*args, **kwargs):
+        stream = sig.bind_partial(*args, **kwargs).arguments.get("stream")
+        if stream is None:
+            return fn(*args, **kwargs)
+        import torch
+        with torch.cuda.stream(stream):
+            return fn(*args, **kwargs)
+    return wrapper
+
+
 def _stream_ptr(torch, stream) -> int:
     s = stream if stream is not None else torch.cuda.current_stream()
     return int(s.cuda_stream)
@@ -261,6 +282,7 @@ def cetra_profile_read(reset: bool = True):
 CETRA_PROBE_FFMA2, CETRA_PROBE_FADD2, CETRA_PROBE_LDS64 = 0, 1, 2
 
 
+@_on_stream
 def cetra_peak_probe(kind: int, iters: int = 20000, stream=None):
     """(units per clock per SM, units per second) of one of the probed instructions; synchronises the stream."""
     torch = _torch()
@@ -290,6 +312,7 @@ class LinearResult:
     stats: object          # [B][J][pitch][2] (S_wmm, S_wmf) or None
 
 
+@_on_stream
 def cetra_linear_search(times, flux, flux_err, durations, t0_start: float, t0_stride: float, n_t0: int, template,
                         want_grids: bool = True, want_stats: bool = False, workspace=None,
                         stream=None) -> LinearResult:
@@ -343,6 +366,7 @@ def peaks_to_numpy(peaks) -> np.ndarray:
     return np.ascontiguousarray(arr).view(PEAK_DTYPE).reshape(arr.shape[:-1])
 
 
+@_on_stream
 def cetra_periodic_search(depth, depth_var, dlogL, t0_start: float, t0_stride: float, durations, periods,
                           dur_lo=None, dur_hi=None, workspace=None, stream=None):
     """Returns a CUDA int32 tensor [B][K][8] holding cetra_peak records (see peaks_to_numpy)."""
@@ -374,6 +398,7 @@ def cetra_periodic_search(depth, depth_var, dlogL, t0_start: float, t0_stride: f
     return peaks
 
 
+@_on_stream
 def cetra_periodic_search_stats(stats, n_t0: int, t0_start: float, t0_stride: float, durations, periods,
                                 dur_lo=None, dur_hi=None, workspace=None, stream=None):
     torch = _torch()
@@ -409,6 +434,7 @@ def cetra_search_batched_workspace_bytes(times, n_lc: int, lc_chunk: int, durati
                                                         _grid(t0_start, t0_stride, n_t0), int(n_template), int(n_per)))
 
 
+@_on_stream
 def cetra_search_batched(times, flux, flux_err, durations, t0_start: float, t0_stride: float, n_t0: int, template,
                          periods, dur_lo=None, dur_hi=None, lc_chunk: int = 0, workspace=None, peaks=None,
                          stream=None):
@@ -438,6 +464,7 @@ def cetra_search_batched(times, flux, flux_err, durations, t0_start: float, t0_s
     return peaks
 
 
+@_on_stream
 def cetra_search_batched_templates(times, flux, flux_err, durations, t0_start: float, t0_stride: float, n_t0: int,
                                    templates, periods, dur_lo=None, dur_hi=None, lc_chunk: int = 0, workspace=None,
                                    stream=None):
@@ -479,6 +506,7 @@ def cetra_search_batched_host_workspace_bytes(times, n_lc: int, lc_chunk: int, d
                                                              int(n_per)))
 
 
+@_on_stream
 def cetra_search_batched_host(times, flux_host, flux_err_host, durations, t0_start: float, t0_stride: float,
                               n_t0: int, template, periods, dur_lo=None, dur_hi=None, lc_chunk: int = 0,
                               workspace=None, peaks_host=None, device=None, stream=None) -> np.ndarray:
@@ -520,6 +548,18 @@ def cetra_search_batched_host(times, flux_host, flux_err_host, durations, t0_sta
 
 
 # ----------------------------------------------------------------------- setup and follow-up steps
+def cetra_resample_template(model, n_template: int = 1024) -> np.ndarray:
+    """Supplied transit model -> n_template-sample search template by linear interpolation; host-side."""
+    lib = load_library()
+    model = np.ascontiguousarray(model, dtype=np.float32)
+    out = np.empty(int(n_template), dtype=np.float32)
+    lib.cetra_resample_template.restype = ctypes.c_int
+    lib.cetra_resample_template.argtypes = [ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p, ctypes.c_int32]
+    _check(lib.cetra_resample_template(model.ctypes.data, model.shape[0], out.ctypes.data, out.shape[0]),
+           "cetra_resample_template")
+    return out
+
+
 def cetra_median_cadence(times) -> float:
     """Default resample cadence: host-only helper of the library."""
     times = _f64(times)
@@ -538,6 +578,7 @@ def cetra_resample_grid(times, cadence: float = 0.0, pad_days: float = 0.0):
     return t_start.value, c.value, int(n_out.value)
 
 
+@_on_stream
 def cetra_resample(times_dev, flux, flux_err, t_start: float, cadence: float, n_out: int, workspace=None,
                    stream=None):
     """Irregular light curves [B][N_in] (or [N_in]) sharing `times_dev` -> (flux, flux_err) on the regular grid."""
@@ -570,6 +611,7 @@ class MonotransitResult:
     profile_j: object
 
 
+@_on_stream
 def cetra_monotransit_search(depth, depth_var, dlogL, t0_start: float, t0_stride: float, durations, n_peaks: int,
                              excl: float = 1.0, want_profile: bool = False, workspace=None,
                              stream=None) -> MonotransitResult:
@@ -607,6 +649,7 @@ def events_to_numpy(events) -> np.ndarray:
     return a.view(EVENT_DTYPE).reshape(a.shape[:-1])
 
 
+@_on_stream
 def cetra_mask_transits(times_dev, flux, period, t0, duration, width: float = 1.0, workspace=None, stream=None):
     """Set the samples within width*D/2 of a transit mid-time to NaN, in place; returns the
     per-curve count of nullified samples as an int32 CUDA tensor."""

@@ -221,6 +221,21 @@ int cetra_median_cadence(const double *times_host, int64_t n, double *cadence) {
     return CETRA_OK;
 }
 
+int cetra_resample_template(const float *model_host, int32_t n_model, float *template_host, int32_t n_template) {
+    if (!model_host || !template_host || n_model < 2 || n_template < 2) return CETRA_ERR_INVALID_ARG;
+    // "resampled to a user-defined number of samples using simple linear interpolation"; both ends kept
+    const double step = static_cast<double>(n_model - 1) / static_cast<double>(n_template - 1);
+    for (int32_t m = 0; m < n_template; ++m) {
+        const double u = static_cast<double>(m) * step;
+        int32_t i0 = static_cast<int32_t>(floor(u));
+        if (i0 > n_model - 2) i0 = n_model - 2;
+        const double fr = u - static_cast<double>(i0);
+        const double a = static_cast<double>(model_host[i0]), b = static_cast<double>(model_host[i0 + 1]);
+        template_host[m] = static_cast<float>(a + (b - a) * fr);
+    }
+    return CETRA_OK;
+}
+
 int cetra_resample_grid(const double *times_host, int64_t n, double cadence, double pad_days, double *t_start,
                         double *cadence_out, int64_t *n_out) {
     if (!times_host || !t_start || !cadence_out || !n_out || n < 2 || !(pad_days >= 0.0) || !std::isfinite(pad_days))

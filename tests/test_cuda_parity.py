@@ -434,6 +434,63 @@ def test_batched_equals_single_and_host_variant(torch_cuda, cetra, oracle_mod):
         assert_periodic_parity(pk[b], orc, cell, what=f"batch lc {b}")
 
 
+def test_large_time_origin(torch_cuda, cetra, oracle_mod):
+    """Times as BJD - 2 457 000 (origin ~ 3e3 d) and as full BJD: the sample times are then only regular to the FP64
+    rounding of the origin, the float32 `t0` of a record resolves 20 s / 0.25 d, and i_t0 stays exact (cetra.h):
+    the records match the oracle's on the shifted times, and the indices those of the search with origin 0."""
+    p = _problem(1)
+    periods = p.periods[::5]
+    flux, err = _dev(torch_cuda, p.flux), _dev(torch_cuda, p.flux_err)
+    base = cetra.peaks_to_numpy(cetra.cetra_search_batched(p.times, flux[None], err[None], p.durations, p.t0_start,
+                                                           p.t0_stride, p.n_t0, p.template, periods))[0]
+    for origin in (3456.0, 2458849.5):
+        times = origin + np.arange(p.n) * p.cadence
+        c = (times[-1] - times[0]) / (p.n - 1)                   # the cadence the library derives from these times
+        pk = cetra.peaks_to_numpy(cetra.cetra_search_batched(times, flux[None], err[None], p.durations, times[0], c,
+                                                             p.n_t0, p.template, periods))[0]
+        o = oracle_mod.linear_search(times, p.flux, p.flux_err, p.durations, times[0], c, p.n_t0, p.template)
+        orc = oracle_mod.periodic_search(o, times[0], c, p.durations, periods)
+        assert_periodic_parity(pk, orc, lambda k, j, ph: oracle_mod.periodic_cell(o, c, periods[k], j, ph),
+                               what=f"origin {origin}")
+        same = (pk["i_t0"] == base["i_t0"]) & (pk["j_dur"] == base["j_dur"])       # rounding of the shifted times may
+        assert same.mean() >= 0.9                                                    # move a near-tie, not more
+        exact = times[0] + pk["i_t0"].astype(np.float64) * c
+        assert np.array_equal(pk["t0"], exact.astype(np.float32))                      # float32 of the exact time ...
+        assert np.abs(pk["t0"].astype(np.float64) - exact).max() > 1e-5               # ... which is coarser than a sample
+
+
+def test_search_on_a_side_stream(torch_cuda, cetra):
+    """Every wrapper takes `stream=`: workspace, outputs and input copies are then made on that stream (binding
+    _on_stream).  A search enqueued on a side stream, behind a long kernel on that stream, with non-contiguous inputs,
+    gives the records of the same search on the default stream bit for bit."""
+    from cetra_synth import make_survey_batch
+    torch = torch_cuda
+    p = make_survey_batch(n_lc=6, n_periods=400)
+    wide_f = torch.from_numpy(np.ascontiguousarray(np.repeat(p.flux, 2, axis=1))).cuda()
+    wide_e = torch.from_numpy(np.ascontiguousarray(np.repeat(p.flux_err, 2, axis=1))).cuda()
+    flux, err = wide_f[:, ::2], wide_e[:, ::2]                   # strided views: the wrapper must copy them
+    assert not flux.is_contiguous()
+    args = (p.times, flux, err, p.durations, p.t0_start, p.t0_stride, p.n_t0, p.template, p.periods)
+    ref = cetra.peaks_to_numpy(cetra.cetra_search_batched(*args))
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    busy = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    with torch.cuda.stream(side):
+        for _ in range(20):
+            busy.add_(1)                                         # the side stream is busy when the search is enqueued
+    got = cetra.cetra_search_batched(*args, stream=side)
+    churn = [torch.full((1 << 20,), 7, dtype=torch.int32, device="cuda") for _ in range(32)]   # default-stream allocations
+    side.synchronize()
+    torch.cuda.synchronize()
+    assert np.array_equal(cetra.peaks_to_numpy(got).view(np.uint8), ref.view(np.uint8))
+    lin = cetra.cetra_linear_search(*args[:8], want_stats=True, stream=side)
+    side.synchronize()
+    lin0 = cetra.cetra_linear_search(*args[:8], want_stats=True)
+    torch.cuda.synchronize()
+    assert torch.equal(lin.stats, lin0.stats) and torch.equal(torch.nan_to_num(lin.depth), torch.nan_to_num(lin0.depth))
+    del churn
+
+
 def test_template_sequence_equals_one_search_per_template(torch_cuda, cetra, oracle_mod):
     """a sequence of impact parameters.  Every template's records are bit-identical to a search
     with that template alone, and the grazing template is checked against the oracle."""

@@ -130,3 +130,16 @@ def test_peak_record_layout(cetra):
     assert ctypes.sizeof(cetra_peak) == 32 == cetra.PEAK_DTYPE.itemsize
     for name, _ in cetra_peak._fields_:
         assert getattr(cetra_peak, name).offset == cetra.PEAK_DTYPE.fields[name][1]
+
+
+def test_resample_template_host_helper_matches_the_oracle(cetra, oracle_mod):
+    """cetra_resample_template (host-side setup helper) against the oracle's linear interpolation."""
+    from cetra_synth import tabulate_template
+    dense = tabulate_template(20001)                              # a densely sampled model, as the paper ships
+    for m in (64, 1024, 4096):
+        got = cetra.cetra_resample_template(dense, m)
+        want = oracle_mod.resample_template(dense.astype(np.float32).astype(np.float64), m)
+        assert got.dtype == np.float32 and got.shape == (m,)
+        assert np.array_equal(got, want.astype(np.float32)) or np.abs(got - want).max() <= 6e-8
+    with pytest.raises(cetra.CetraError):
+        cetra.cetra_resample_template(dense[:1], 8)

@@ -83,6 +83,22 @@ def test_resample_assigns_to_the_nearest_output_point(oracle_mod):
     assert np.isnan(of[3])                     # -0.51 c is before the grid: dropped
 
 
+def test_resample_template_is_numpy_interp_and_keeps_a_linear_model(oracle_mod):
+    """the supplied model is resampled "using simple linear interpolation".  Pins: numpy.interp on the
+    same positions; a straight-line model is reproduced exactly at every output sample; the same sample count is the
+    identity; the end samples are kept."""
+    rng = np.random.default_rng(4)
+    model = np.cumsum(rng.normal(size=317))
+    for n_out in (2, 5, 317, 1024):
+        got = oracle_mod.resample_template(model, n_out)
+        want = np.interp(np.linspace(0.0, 316.0, n_out), np.arange(317.0), model)
+        assert np.allclose(got, want, rtol=0, atol=1e-12 * np.abs(model).max())
+        assert got[0] == model[0] and abs(got[-1] - model[-1]) <= 1e-12 * abs(model[-1])
+    assert np.allclose(oracle_mod.resample_template(model, 317), model, rtol=0, atol=1e-12 * np.abs(model).max())
+    line = 3.0 - 0.25 * np.arange(41.0)
+    assert np.allclose(oracle_mod.resample_template(line, 1001), np.linspace(line[0], line[-1], 1001), rtol=0, atol=1e-12)
+
+
 def test_median_cadence_is_numpy_median_of_differences(oracle_mod):
     rng = np.random.default_rng(3)
     t = np.cumsum(rng.choice([1.0, 1.0, 1.0, 2.0, 7.5], size=1001) * 2.0 / 1440.0)
