@@ -529,6 +529,43 @@ def run_configs(args):
                           frac_hbm=moved / (rs_ms * 1e-3) / 1e9 / peaks_hw["hbm_gbs"])), flush=True)
 
 
+# --------------------------------------------------------- tensor-core variant of the windowed sums (diagnostic)
+def run_tc_probe(args):
+    """SURVEY.md §8(f) 4 / north_star: the tensor-core banded-correlation variant "must beat the CUDA-core version".
+    For window lengths spanning the config-2 durations: linear_search_kernel (64 survey curves, one duration, statistics
+    only) against cetra_tc_correlation_probe (mma.sync TF32 Toeplitz products, same number of outputs), both as
+    (t0, point) template evaluations per second; the 3xTF32 split is what the 1e-5 parity bar needs."""
+    import torch
+    import paper_2503_20875_b200 as cetra
+    from cetra_synth import make_survey_batch
+    torch.cuda.set_device(0)
+    p = make_survey_batch(n_lc=args.n_lc, lc_range=(0, args.n_lc))
+    flux, err = torch.from_numpy(p.flux).cuda(), torch.from_numpy(p.flux_err).cuda()
+    for k_taps in (17, 61, 121, 241, 361):
+        dur = np.array([(k_taps - 0.5) * p.cadence])                 # a window of exactly k_taps samples
+        for _ in range(3):
+            cetra.cetra_linear_search(p.times, flux, err, dur, p.t0_start, p.t0_stride, p.n_t0, p.template,
+                                      want_grids=False, want_stats=True)
+        torch.cuda.synchronize()
+        cetra.cetra_profile_enable(True)
+        for _ in range(20):
+            cetra.cetra_linear_search(p.times, flux, err, dur, p.t0_start, p.t0_stride, p.n_t0, p.template,
+                                      want_grids=False, want_stats=True)
+        torch.cuda.synchronize()
+        pr = cetra.cetra_profile_read()
+        cetra.cetra_profile_enable(False)
+        cuda_ms = pr["linear_ms"] / pr["linear_launches"]
+        n_out = args.n_lc * p.n_t0
+        line = dict(workload="windowed sums of one duration, %d curves x %d t0 cells" % (args.n_lc, p.n_t0),
+                    taps=k_taps, cuda_core=dict(kernel="linear_search_kernel", ms=cuda_ms,
+                                                evals_per_s=n_out * k_taps / (cuda_ms * 1e-3)))
+        for split in (True, False):
+            r = cetra.cetra_tc_correlation_probe(n_out, k_taps, split=split, reps=20)
+            line["tensor_3xtf32" if split else "tensor_1xtf32"] = r
+        line["tensor_over_cuda_core"] = line["tensor_3xtf32"]["evals_per_s"] / line["cuda_core"]["evals_per_s"]
+        print(json.dumps(line), flush=True)
+
+
 def spawn_command(n_gpus: int, port: int, argv):
     """The torchrun command `python bench.py --gpus N` runs itself under when it was not started by torchrun."""
     return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n_gpus}",
@@ -541,7 +578,7 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--workload", default="sector", choices=["sector", "survey", "configs"])
+    ap.add_argument("--workload", default="sector", choices=["sector", "survey", "configs", "tc-probe"])
     ap.add_argument("--cfgs", default="1,2,3,4", help="--workload configs: which BASELINE configs to time")
     ap.add_argument("--n-lc", type=int, default=64, help="light curves per GPU per step (survey: per slice)")
     ap.add_argument("--lc-chunk", type=int, default=0, help="light curves resident at a time (0 = library default)")
@@ -564,6 +601,8 @@ def main():
         run_reference(args, rank)
     elif args.workload == "survey":
         run_survey(args)
+    elif args.workload == "tc-probe":
+        run_tc_probe(args)
     elif args.workload == "configs":
         run_configs(args)
     else:

@@ -34,6 +34,7 @@ EXPORTED_SYMBOLS = (
     "cetra_search_batched_templates_workspace_bytes",
     "cetra_search_batched_host_workspace_bytes", "cetra_search_batched_host",
     "cetra_profile_enable", "cetra_profile_read", "cetra_peak_probe_workspace_bytes", "cetra_peak_probe",
+    "cetra_tc_correlation_probe_workspace_bytes", "cetra_tc_correlation_probe",
     "cetra_resample_template", "cetra_median_cadence", "cetra_resample_grid", "cetra_resample_workspace_bytes", "cetra_resample",
     "cetra_monotransit_workspace_bytes", "cetra_monotransit_search",
     "cetra_mask_workspace_bytes", "cetra_mask_transits",
@@ -293,6 +294,27 @@ def cetra_peak_probe(kind: int, iters: int = 20000, stream=None):
     _check(lib.cetra_peak_probe(int(kind), int(iters), ctypes.byref(a), ctypes.byref(b), ws.data_ptr(), ws.numel(),
                                 _stream_ptr(torch, stream)), "cetra_peak_probe")
     return a.value, b.value
+
+
+@_on_stream
+def cetra_tc_correlation_probe(n_out: int, n_taps: int, split: bool = True, reps: int = 20, stream=None):
+    """The measured tensor-core variant of the windowed sums (cetra.h): dict(ms, evals_per_s, err_wmf, err_wmm)."""
+    torch = _torch()
+    lib = load_library()
+    lib.cetra_tc_correlation_probe_workspace_bytes.restype = ctypes.c_size_t
+    lib.cetra_tc_correlation_probe_workspace_bytes.argtypes = [ctypes.c_int64, ctypes.c_int32]
+    lib.cetra_tc_correlation_probe.restype = ctypes.c_int
+    lib.cetra_tc_correlation_probe.argtypes = [ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
+                                               ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double),
+                                               ctypes.POINTER(ctypes.c_double), ctypes.c_void_p, ctypes.c_size_t,
+                                               ctypes.c_void_p]
+    nbytes = int(lib.cetra_tc_correlation_probe_workspace_bytes(int(n_out), int(n_taps)))
+    ws = _workspace(torch, nbytes, torch.device("cuda", torch.cuda.current_device()))
+    ms, ef, ew = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+    _check(lib.cetra_tc_correlation_probe(int(n_out), int(n_taps), 1 if split else 0, int(reps), ctypes.byref(ms),
+                                          ctypes.byref(ef), ctypes.byref(ew), ws.data_ptr(), ws.numel(),
+                                          _stream_ptr(torch, stream)), "cetra_tc_correlation_probe")
+    return dict(ms=ms.value, evals_per_s=float(n_out) * n_taps / (ms.value * 1e-3), err_wmf=ef.value, err_wmm=ew.value)
 
 
 def cetra_linear_workspace_bytes(times, n_lc: int, durations, t0_start, t0_stride, n_t0, n_template: int) -> int:

@@ -15,7 +15,7 @@ _ROOT = os.path.dirname(_PKG)
 CSRC = os.path.join(_PKG, "csrc")
 INCLUDE = os.path.join(_ROOT, "include")
 LIB_PATH = os.environ.get("CETRA_LIB_PATH") or os.path.join(_PKG, "libcetra_b200.so")
-SOURCES = ["cetra_api.cu", "linear_search.cu", "periodic_search.cu", "fold_pair.cu", "fold_stream.cu", "setup_steps.cu", "peak_probe.cu"]
+SOURCES = ["cetra_api.cu", "linear_search.cu", "periodic_search.cu", "fold_pair.cu", "fold_stream.cu", "setup_steps.cu", "peak_probe.cu", "tc_probe.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-shared", "-Xcompiler", "-fPIC", "--threads", "0",
