@@ -40,22 +40,8 @@ namespace {
 #endif
 constexpr int kPairS = CETRA_PAIR_S;                  // |shift| up to which the two periods share one register window
 constexpr int kPairFar = 2 * kPairS + 1;   // class of the epochs whose periods gather separately
-constexpr int kPairMaxM = 64;              // cap on the centring shift (the header in front of the row absorbs -m)
 static_assert(kGrpHeaderBytes >= 16 + (kGrpThreads / 32) * 512 && kGrpHeaderBytes >= 8 * (kPairMaxM + kPairS + 1), "cells before the row start are read (and discarded)");
 static_assert(kStatsPad >= 32 * (kGrpG + 2) + kPairS + 1 + kPairMaxM, "cells past the last t0 cell are read as zeros");
-
-// One epoch of a pair whose windows are S cells apart (S < 0: the longer period's cells come first).
-template <int S, int G>
-__device__ __forceinline__ void fold_epoch_c(float2 (&acc)[kGrpT][G], uint32_t ptr) {
-    constexpr int A = S < 0 ? -S : S;
-    float2 c[G + A];
-#pragma unroll
-    for (int i = 0; i < G + A; ++i) c[i] = lds_cell(ptr + 8u * i);
-#pragma unroll
-    for (int g = 0; g < G; ++g) acc[0][g] = add2(acc[0][g], c[g + (S < 0 ? A : 0)]);
-#pragma unroll
-    for (int g = 0; g < G; ++g) acc[1][g] = add2(acc[1][g], c[g + (S > 0 ? A : 0)]);
-}
 
 // The epochs `mk` (bit t = epoch eb + t) of one block, all of shift S: a straight-line loop over the set bits.
 // ew holds the block's (off_0, off_1 - m) words; the next epoch's word is fetched while the current one is folded.
@@ -297,13 +283,7 @@ __global__ void __launch_bounds__(kGrpThreads, 1) fold_pair_argmax_kernel(const 
                     const int tk = kk[0]; kk[0] = kk[1]; kk[1] = tk;
                 }
                 // centring: half of the largest offset difference of the pair (reached at the last epoch)
-                int m = 0;
-                if (gp.n_phase[0] > 0 && gp.n_phase[1] > 0) {
-                    // any m gives the same records; this one halves the average window
-                    const float e_last = static_cast<float>(P.n_t0 - 1) / static_cast<float>(gp.r[0]);
-                    const float half = 0.5f * e_last * static_cast<float>(gp.r[1] - gp.r[0]);
-                    m = half < static_cast<float>(kPairMaxM) ? static_cast<int>(half + 0.5f) : kPairMaxM;
-                }
+                const int m = gp.n_phase[0] > 0 && gp.n_phase[1] > 0 ? centring_shift(gp.r[0], gp.r[1], P.n_t0) : 0;
                 // phases to cover: [0, n_phase_0) of period 0 from p0 on, [0, n_phase_1) of period 1 from p0 - m on
                 const int n_need = max(gp.n_phase[0], gp.n_phase[1] > 0 ? gp.n_phase[1] + m : 0);
                 // The period's best so far (over the rows already folded, by any CTA) dismisses most cells without a

@@ -15,9 +15,12 @@ constexpr size_t kGrpHeaderBytes = 16 + (kGrpThreads / 32) * 64 * 8;   // barrie
 // (640 threads keep the 96-register budget the two-period register window needs).
 constexpr int kStrThreads = 640;
 constexpr int kStrUnitPeriods = (kStrThreads / 32 - 1) * kGrpT;
-constexpr int kStrStagesLog2 = 3;
+#ifndef CETRA_STR_STAGES_LOG2
+#define CETRA_STR_STAGES_LOG2 2
+#endif
+constexpr int kStrStagesLog2 = CETRA_STR_STAGES_LOG2;
 constexpr int kStrStages = 1 << kStrStagesLog2;
-constexpr size_t kStrHeaderBytes = 512;                                  // barriers + stage descriptors
+constexpr size_t kStrHeaderBytes = 8192;                                 // barriers, stage descriptors, per-warp epoch words
 static_assert(kStatsPad >= 32 * (kGrpG + 2) + kGrpS + 1, "the widest (last) pass may read 32*(G+2)+S cells past the last t0 cell");
 
 struct PeriodicParams {
