@@ -394,12 +394,34 @@ linear_search_kernel(const __grid_constant__ LinearParams P) {
 }
 
 // ------------------------------------------------------------------------------- L2 + L3, off-grid t0
-// The t0 grid does not sit on the sample grid (the paper's default stride is 1 % of the shortest duration,
-// PAPER.md:87), so the template sample of a (cell, sample) pair cannot be tabulated per duration: one thread
-// owns one cell and derives x = (n c - t_i)/D + 1/2 and the nearest-neighbour index per sample in FP64 (R25),
-// exactly rounded operation by operation.  Bound by the FP64 pipe (one IEEE division per template eval);
-// neighbouring lanes read the same samples (the stride is far below the cadence), so loads broadcast.
-__global__ void __launch_bounds__(128) linear_general_kernel(const __grid_constant__ GeneralParams P) {
+// A t0 grid off the sample grid whose stride is not a small rational multiple of the cadence (those take the residue
+// classes of linear_search_kernel): the template sample of a (cell, sample) pair cannot be tabulated, so one thread
+// owns one cell.  The definition (R25) derives x = (n c - t_i)/D + 1/2 and idx = floor(x (M-1) + 1/2) per pair with
+// five rounded FP64 operations, one of them a division.  This kernel gets the same index from a position that is
+// STEPPED: with n = n_c + k around the cell's nearest sample n_c,
+//     pos(k) = x(M-1) + 1/2 = k alpha + beta,   alpha = c (M-1)/D,   beta = (n_c c - t_i)(M-1)/D + (M-1)/2 + 1/2,
+// beta from one exact FMA per cell, pos re-anchored in FP64 every 64 samples and advanced in 32.32 fixed point in
+// between (two integer adds per sample).  pos differs from the position the definition's rounded sequence produces by
+// at most eps (host: build_linear_plan), so floor(pos) is the definition's index unless pos lies within eps of an
+// integer; the kernel tracks the smallest distance of a block's positions from an integer (one IMNMX per sample, on a
+// representation shifted by eps so that the distance is the low word) and recomputes a block with the exact sequence
+// (r25_index) when that distance is below 2 eps.  The window edges (x = 0, x = 1) are decided the same way: from pos
+// when it is further than eps from the edge, exactly otherwise.
+// Neighbouring lanes read the same samples (the stride is far below the cadence), so those loads broadcast; the
+// template (m, m^2) pairs are gathered from shared memory.
+constexpr int kGenThreads = 128;          // 256 threads, 64 threads and deeper unrolling measured the same or slower
+constexpr int kGenBlock = 64;            // samples between FP64 re-anchorings of the position (and per FP32 partial sum)
+
+template <bool TPL_SMEM>
+__global__ void __launch_bounds__(kGenThreads) linear_general_kernel(const __grid_constant__ GeneralParams P) {
+    extern __shared__ __align__(16) float2 s_tpl2[];   // (m, m^2) per template sample, one spare entry
+    if (TPL_SMEM) {
+        for (int t = threadIdx.x; t <= P.n_tpl; t += kGenThreads) {
+            const float m = t < P.n_tpl ? P.tpl[t] : 0.f;
+            s_tpl2[t] = make_float2(m, m * m);
+        }
+        __syncthreads();
+    }
     const long long i = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x;
     const int j = blockIdx.y;
     const long long lc = blockIdx.z;
@@ -409,30 +431,90 @@ __global__ void __launch_bounds__(128) linear_general_kernel(const __grid_consta
         return;
     }
     const double D = P.durations[j], c = P.cadence;
-    const double ti = __dadd_rn(P.delta, __dmul_rn(static_cast<double>(i), P.stride));   // t_i - times[0]
-    const double half = __dmul_rn(0.5, D);
-    long long lo = static_cast<long long>(floor(__ddiv_rn(__dsub_rn(ti, half), c))) - 1;  // superset of the window
-    long long hi = static_cast<long long>(floor(__ddiv_rn(__dadd_rn(ti, half), c))) + 2;
-    lo = lo < 0 ? 0 : lo;
-    hi = hi > P.n - 1 ? P.n - 1 : hi;
     const double Mm1 = static_cast<double>(P.n_tpl - 1);
-    const float2 *x_row = P.wfw + lc * P.lc_pitch;
+    const double ti = __dadd_rn(P.delta, __dmul_rn(static_cast<double>(i), P.stride));   // t_i - times[0], as R25 forms it
+    // nearest sample and the stepped position
+    const long long nc = __double2ll_rn(ti / c);
+    const double d0 = fma(static_cast<double>(nc), c, -ti);                 // n_c c - t_i, one rounding
+    const double g = Mm1 / D;
+    const double alpha = c * g;
+    const double beta = fma(d0, g, 0.5 * Mm1 + 0.5);
+    const double eps = P.eps_scale / D + P.eps_abs;
+    // window: samples with 1/2 <= pos <= M - 1/2 (x in [0, 1], both edges included, R2), clipped to the data
+    const double inv_alpha = 1.0 / alpha;
+    long long kf = static_cast<long long>(ceil((0.5 - beta) * inv_alpha));
+    long long kl = static_cast<long long>(floor((Mm1 + 0.5 - beta) * inv_alpha));
+    {
+        // an edge is decided by the stepped position when that is further than eps from it, exactly otherwise
+        const double pf0 = fma(static_cast<double>(kf - 1), alpha, beta), pf1 = fma(static_cast<double>(kf), alpha, beta);
+        if (!(pf0 < 0.5 - eps && pf1 > 0.5 + eps)) {
+            long long k = kf - 2;
+            for (; k <= kf + 2; ++k)
+                if (r25_index(nc + k, ti, c, D, Mm1) >= 0) break;
+            kf = k;                                                          // kf + 3 when none: an empty window
+        }
+        const double pl0 = fma(static_cast<double>(kl), alpha, beta), pl1 = fma(static_cast<double>(kl + 1), alpha, beta);
+        if (!(pl0 < Mm1 + 0.5 - eps && pl1 > Mm1 + 0.5 + eps)) {
+            long long k = kl + 2;
+            for (; k >= kl - 2; --k)
+                if (r25_index(nc + k, ti, c, D, Mm1) >= 0) break;
+            kl = k;
+        }
+    }
+    kf = kf < -nc ? -nc : kf;
+    kl = kl > P.n - 1 - nc ? P.n - 1 - nc : kl;
+    // fixed point: 32.32, positions shifted up by eps (then "within eps of an integer" reads "low word < 2 eps")
+    const double two32 = 4294967296.0;
+    const unsigned long long alpha_fx = static_cast<unsigned long long>(__double2ll_rn(alpha * two32));
+    const double eps_c = eps < 0.24 ? eps : 0.24;
+    const unsigned int two_eps_fx = static_cast<unsigned int>(2.0 * eps_c * two32) + 2u;
+    const bool all_exact = !(eps < 0.24) || !(alpha < 1.0e9);               // no usable margin: every block exactly
+    const float2 *x_row = P.wfw + lc * P.lc_pitch + nc;
     float s_mf = 0.f, s_mm = 0.f;                       // two-level FP32 sums, as in linear_search_kernel
-    for (long long n0 = lo; n0 <= hi; n0 += 64) {
+    unsigned int n_exact = 0;
+    for (long long kb = kf; kb <= kl; kb += kGenBlock) {
+        const int cnt = static_cast<int>(kl - kb + 1 < kGenBlock ? kl - kb + 1 : kGenBlock);
+        const float2 *xp = x_row + kb;
         float a_mf = 0.f, a_mm = 0.f;
-        const long long n1 = n0 + 63 < hi ? n0 + 63 : hi;
-        for (long long nn = n0; nn <= n1; ++nn) {
-            const double x = __dadd_rn(__ddiv_rn(__dsub_rn(__dmul_rn(static_cast<double>(nn), c), ti), D), 0.5);
-            if (x >= 0.0 && x <= 1.0) {
-                const float m = __ldg(P.tpl + static_cast<int>(floor(__dadd_rn(__dmul_rn(x, Mm1), 0.5))));
-                const float2 s = __ldg(x_row + nn);
-                a_mf = fmaf(m, s.x, a_mf);              // S_wmf += m * (w f)
-                a_mm = fmaf(m * m, s.y, a_mm);          // S_wmm += m^2 * w
+        unsigned int nearest = 0xffffffffu;
+        if (!all_exact) {
+            const double pos0 = fma(static_cast<double>(kb), alpha, beta) + eps_c;
+            unsigned long long fx = static_cast<unsigned long long>(__double2ll_rn(pos0 * two32));
+#pragma unroll 4
+            for (int t = 0; t < cnt; ++t) {
+                const unsigned int idx = static_cast<unsigned int>(fx >> 32);
+                nearest = min(nearest, static_cast<unsigned int>(fx));
+                const float2 s = __ldg(xp + t);
+                float2 m2;
+                if (TPL_SMEM) {
+                    m2 = s_tpl2[idx];
+                } else {
+                    const float m = __ldg(P.tpl + (idx < static_cast<unsigned int>(P.n_tpl) ? idx : P.n_tpl - 1));
+                    m2 = make_float2(m, m * m);
+                }
+                a_mf = fmaf(m2.x, s.x, a_mf);            // S_wmf += m * (w f)
+                a_mm = fmaf(m2.y, s.y, a_mm);            // S_wmm += m^2 * w
+                fx += alpha_fx;
             }
+        }
+        if (all_exact || nearest < two_eps_fx) {
+            // some position of the block is within rounding of an index step: the definition's own sequence
+            a_mf = 0.f; a_mm = 0.f;
+            for (int t = 0; t < cnt; ++t) {
+                const int idx = r25_index(nc + kb + t, ti, c, D, Mm1);
+                if (idx >= 0) {
+                    const float m = __ldg(P.tpl + idx);
+                    const float2 s = __ldg(xp + t);
+                    a_mf = fmaf(m, s.x, a_mf);
+                    a_mm = fmaf(m * m, s.y, a_mm);
+                }
+            }
+            n_exact += cnt;
         }
         s_mf += a_mf;
         s_mm += a_mm;
     }
+    if (n_exact && P.exact_evals) atomicAdd(P.exact_evals, static_cast<unsigned long long>(n_exact));
     const bool null_cell = !(s_mm > 0.f);               // no observation in the window
     const float nanv = __int_as_float(0x7fc00000);
     const float depth = null_cell ? nanv : s_mf / s_mm;
@@ -479,6 +561,17 @@ int build_linear_plan(const double *times_host, int64_t n, int32_t n_lc, const d
         for (int j = 0; j < n_dur; ++j) {
             if (!(durations_host[j] > 0.0) || !std::isfinite(durations_host[j])) return CETRA_ERR_INVALID_ARG;
             G.durations[j] = durations_host[j];
+        }
+        // How far the stepped position (see linear_general_kernel) can lie from the one the definition's rounded FP64
+        // sequence produces, in template samples: the sequence itself (3 T 2^-53 (M-1)/D + 4 M 2^-53, T the largest
+        // time magnitude), the stepping (FMA anchor, alpha's rounding over <= 64 steps, the 32.32 conversion and 64
+        // fixed-point steps: < 2^-26); doubled.
+        {
+            double t_max = std::max(fabs(pl->geo.delta), fabs(pl->geo.delta + static_cast<double>(grid.n_t0) * pl->geo.stride));
+            t_max = std::max(t_max, static_cast<double>(n) * pl->geo.cadence);
+            const double ulp = 1.1102230246251565e-16;
+            G.eps_scale = 2.0 * 6.0 * t_max * ulp * static_cast<double>(n_template - 1);
+            G.eps_abs = 2.0 * (64.0 * static_cast<double>(n_template) * ulp + 1.4901161193847656e-08);
         }
         pl->P.lc_pitch = G.lc_pitch;
         pl->P.n_lo = 0;
@@ -704,13 +797,20 @@ int run_linear(LinearPlan &pl, const void *flux_dev, const void *flux_err_dev, c
         G.depth = depth_dev; G.var = var_dev; G.dlogL = dlogL_dev;
         G.stats = reinterpret_cast<float2 *>(stats_dev);
         const long long cells = stats_dev ? G.stats_pitch : G.n_t0;
-        const dim3 g(static_cast<unsigned>((cells + 127) / 128), static_cast<unsigned>(G.n_dur),
+        const dim3 g(static_cast<unsigned>((cells + kGenThreads - 1) / kGenThreads), static_cast<unsigned>(G.n_dur),
                      static_cast<unsigned>(n_lc));
         profile_mark(kProfLinear, true, st);
         for (int t = 0; t < T; ++t) {                           // one launch per template of the set
             G.tpl = tpl + static_cast<size_t>(t) * n_template;
             G.row0 = static_cast<long long>(t) * n_lc * G.n_dur;
-            linear_general_kernel<<<g, 128, 0, st>>>(G);
+            const size_t tpl_bytes = sizeof(float2) * (static_cast<size_t>(n_template) + 1);
+            if (tpl_bytes <= 96 * 1024) {                       // (m, m^2) table in shared memory
+                auto k = linear_general_kernel<true>;
+                CETRA_CUDA_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+                k<<<g, kGenThreads, tpl_bytes, st>>>(G);
+            } else {
+                linear_general_kernel<false><<<g, kGenThreads, 0, st>>>(G);
+            }
             CETRA_LAUNCH_CHECK();
         }
         profile_mark(kProfLinear, false, st);

@@ -630,11 +630,18 @@ def test_off_grid_default_stride_takes_the_exact_fallback(torch_cuda, cetra, ora
     print("default-grid worst", worst, "exact evaluations", n_exact)
     assert n_exact > 0
     # a stride that is not a small rational multiple of the cadence takes the per-cell kernel, same bar
+    # (stepped fixed-point positions; cell 0 sits on a sample, so its centre position is exactly on an index step and
+    # that block must take the exact sequence too)
     stride2 = stride * (1.0 + 1.0 / 977.0)
     o2 = oracle_mod.linear_search(p.times, p.flux, p.flux_err, p.durations, t0_start, stride2, 12000, p.template)
+    cetra.cetra_exact_eval_count(reset=True)
     r2 = cetra.cetra_linear_search(p.times, flux, err, p.durations, t0_start, stride2, 12000, p.template)
+    n_exact2 = cetra.cetra_exact_eval_count()
     assert_linear_parity(r2.depth.cpu().numpy(), r2.depth_var.cpu().numpy(), r2.dlogL.cpu().numpy(),
                          o2.depth, o2.depth_var, o2.dlogL, what="config 2 irrational stride")
+    n_evals2 = sum(12000 * (2 * int(d / (2 * (p.times[1] - p.times[0]))) + 1) for d in p.durations)
+    print("irrational stride: exact evaluations", n_exact2, "of about", n_evals2)
+    assert 0 < n_exact2 < 0.01 * n_evals2
     # a whole-sample stride whose START is off the sample grid: a single residue class with a sub-sample offset
     c = p.times[1] - p.times[0]
     for start in (p.times[0] + 0.3 * c, p.times[0] - 100.5 * c):      # the second puts every cell half-way between samples
