@@ -49,12 +49,12 @@ SMEM_BYTES_PER_CLK = 128             # shared-memory crossbar bytes/clk/SM (B300
 # depend on timing), valid for the kernel sources whose hash is `src_sha256`: bench.py hashes the sources it runs
 # and reports `stale: true` (and no traffic) when they differ.
 NCU_FOLD = dict(
-    profile="profiles/r02a_fold_pair_full.md", commit="e202b0a", n_lc=64,
-    src_sha256="32a081b8265e7aa99b2d7294c86fc5ffee8188ad57ae4ce40dc20d30de7c5556",
-    lds_wavefronts=32075992439.0,       # l1tex__data_pipe_lsu_wavefronts_mem_shared.sum (128 B each)
-    dram_bytes=334122240.0 + 14267648.0,  # dram__bytes_read.sum + dram__bytes_write.sum
-    crossbar_pct_under_ncu=90.54,       # ...wavefronts_mem_shared.sum.pct_of_peak_sustained_elapsed
-    duration_ms_under_ncu=121.92,
+    profile="profiles/r02e_fold_pair_full.md", commit="745bae4", n_lc=64,
+    src_sha256="c90a43ac5eb989ac41d614e9fb2c6ad999a757de1969608ca86017f7c8a2eebd",
+    lds_wavefronts=32077297970.0,       # l1tex__data_pipe_lsu_wavefronts_mem_shared.sum (128 B each)
+    dram_bytes=332699648.0 + 12200960.0,  # dram__bytes_read.sum + dram__bytes_write.sum
+    crossbar_pct_under_ncu=90.65,       # ...wavefronts_mem_shared.sum.pct_of_peak_sustained_elapsed
+    duration_ms_under_ncu=121.91,
 )
 FOLD_SOURCES = ("fold_pair.cu", "fold_common.cuh", "periodic_search.cuh", "common.cuh")
 
