@@ -74,6 +74,35 @@ def test_workspace_sizes_scale_with_the_problem(cetra):
     assert cetra.cetra_linear_workspace_bytes(bad, 1, p.durations, p.t0_start, p.t0_stride, p.n_t0, 1024) == 0
 
 
+def test_plan_picks_the_off_grid_path_by_the_stride(cetra):
+    """Host plan logic, seen through the workspace sizes (no device needed): a t0 stride that is a small rational multiple
+    of the cadence (the paper's default, 18 s on 2-min data = 3/20) gets one set of tap tables per residue
+    class; any other stride keeps the per-cell kernel, which needs no tap tables; a template set needs one statistics
+    grid and one set of tap tables per template."""
+    from cetra_synth import make_config
+    p = make_config(2, n_periods=100)
+    c, n_t0 = p.cadence, 30000
+    w = lambda start, stride: cetra.cetra_linear_workspace_bytes(p.times, 1, p.durations, start, stride, n_t0, 1024)
+    on_grid = w(p.times[0], c)
+    classes = w(p.times[0], 0.15 * c)                      # 3/20: 20 classes, each with its own tables and lists
+    general = w(p.times[0], 0.15 * c * (1.0 + 1.0 / 977.0))
+    shifted = w(p.times[0] + 0.3 * c, 2 * c)               # whole-sample stride, off-grid start: one class
+    assert 0 < general < on_grid < shifted < classes
+    assert classes > 3 * on_grid                           # 20 x the tables, with their flags and lists
+    # an almost rational stride is rational only while the cells stay within 1e-6 samples of their class position
+    assert w(p.times[0], 0.15 * c * (1.0 + 1e-12)) == classes
+    assert w(p.times[0], 0.15 * c * (1.0 + 1e-9)) == general
+    lib = cetra.load_library()
+    from paper_2503_20875_b200.binding import cetra_t0_grid, _dp, _f64
+    t, d = _f64(p.times), _f64(p.durations)
+    grid = cetra_t0_grid(p.t0_start, p.t0_stride, p.n_t0)
+    one = lib.cetra_search_batched_templates_workspace_bytes(_dp(t), t.shape[0], 8, 8, _dp(d), d.shape[0], grid, 1024, 1, 100)
+    three = lib.cetra_search_batched_templates_workspace_bytes(_dp(t), t.shape[0], 8, 8, _dp(d), d.shape[0], grid, 1024, 3, 100)
+    assert one == cetra.cetra_search_batched_workspace_bytes(p.times, 8, 8, p.durations, p.t0_start, p.t0_stride, p.n_t0, 1024, 100)
+    stats = 8 * 8 * d.shape[0] * cetra.cetra_stats_pitch(p.n_t0)
+    assert three - one >= 2 * stats and three - one < 2 * stats + (1 << 20)
+
+
 def _call_linear(cetra, times, durations, t0_start, stride, n_t0, n_tpl=64, flux=0x1000, ws=0x10000, ws_bytes=1 << 30,
                  dtype=0, n_lc=1):
     lib = cetra.load_library()
