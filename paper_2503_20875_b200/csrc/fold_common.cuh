@@ -79,19 +79,6 @@ __device__ __forceinline__ void sts_int2(uint32_t addr, int x, int y) {
     asm volatile("st.shared.v2.s32 [%0], {%1, %2};" ::"r"(addr), "r"(x), "r"(y) : "memory");
 }
 
-// One epoch of a two-period group whose offsets differ by D cells: the G + D cells from the smaller offset on are
-// loaded once; period 0 takes cells [0, G), period 1 cells [D, G + D).
-template <int D, int G>
-__device__ __forceinline__ void fold_epoch(float2 (&acc)[kGrpT][G], uint32_t ptr) {
-    float2 c[G + D];
-#pragma unroll
-    for (int i = 0; i < G + D; ++i) c[i] = lds_cell(ptr + 8u * i);
-#pragma unroll
-    for (int g = 0; g < G; ++g) acc[0][g] = add2(acc[0][g], c[g]);
-#pragma unroll
-    for (int g = 0; g < G; ++g) acc[1][g] = add2(acc[1][g], c[g + D]);
-}
-
 constexpr int kPairMaxM = 64;              // cap on the centring shift
 
 // Centring of a pair (r0 <= r1, both searched): half of the largest offset difference, reached at the last epoch.

@@ -8,11 +8,10 @@ namespace cetra {
 // Pair fold (rows resident in shared memory): one warp folds kGrpT neighbouring trial periods together.
 constexpr int kGrpT = 2;             // periods per warp
 constexpr int kGrpG = 11;            // consecutive phases per lane; odd => conflict-free 8-byte LDS at a stride of G cells
-constexpr int kGrpS = 7;             // streamed kernel: largest offset difference of a pair served from one register window
 constexpr int kGrpThreads = 640;     // 20 warps x 96 registers
 constexpr size_t kGrpHeaderBytes = 16 + (kGrpThreads / 32) * 64 * 8;   // barrier, claim slot, epoch words (2 blocks per warp)
-// Streamed fold (rows that do not fit in shared memory): 19 consumer warps + one producer warp, a ring of stages
-// (640 threads keep the 96-register budget the two-period register window needs).
+// Streamed fold (rows that do not fit in shared memory): 19 consumer warps + one producer warp, a ring of stages that
+// hold the windows of a block of epochs each (640 threads keep the 96-register budget of the two-period register window).
 constexpr int kStrThreads = 640;
 constexpr int kStrUnitPeriods = (kStrThreads / 32 - 1) * kGrpT;
 #ifndef CETRA_STR_STAGES_LOG2
@@ -21,7 +20,6 @@ constexpr int kStrUnitPeriods = (kStrThreads / 32 - 1) * kGrpT;
 constexpr int kStrStagesLog2 = CETRA_STR_STAGES_LOG2;
 constexpr int kStrStages = 1 << kStrStagesLog2;
 constexpr size_t kStrHeaderBytes = 8192;                                 // barriers, stage descriptors, per-warp epoch words
-static_assert(kStatsPad >= 32 * (kGrpG + 2) + kGrpS + 1, "the widest (last) pass may read 32*(G+2)+S cells past the last t0 cell");
 
 struct PeriodicParams {
     const float2 *stats;             // [n_lc][n_dur][stats_pitch] (S_wmm, S_wmf), zero in null cells / padding
