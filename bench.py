@@ -49,12 +49,12 @@ SMEM_BYTES_PER_CLK = 128             # shared-memory crossbar bytes/clk/SM (B300
 # depend on timing), valid for the kernel sources whose hash is `src_sha256`: bench.py hashes the sources it runs
 # and reports `stale: true` (and no traffic) when they differ.
 NCU_FOLD = dict(
-    profile="profiles/r02e_fold_pair_full.md", commit="745bae4", n_lc=64,
-    src_sha256="c90a43ac5eb989ac41d614e9fb2c6ad999a757de1969608ca86017f7c8a2eebd",
-    lds_wavefronts=32077297970.0,       # l1tex__data_pipe_lsu_wavefronts_mem_shared.sum (128 B each)
-    dram_bytes=332699648.0 + 12200960.0,  # dram__bytes_read.sum + dram__bytes_write.sum
-    crossbar_pct_under_ncu=90.65,       # ...wavefronts_mem_shared.sum.pct_of_peak_sustained_elapsed
-    duration_ms_under_ncu=121.91,
+    profile="profiles/r02e_fold_pair_full.md", commit="9c3afc6", n_lc=64,
+    src_sha256="7d2b85c78a98cdc2fe2ff350a7ff8c4264e32d289f7b65781ea0f389f99a9de2",
+    lds_wavefronts=32077233385.0,       # l1tex__data_pipe_lsu_wavefronts_mem_shared.sum (128 B each)
+    dram_bytes=332411904.0 + 12120576.0,  # dram__bytes_read.sum + dram__bytes_write.sum
+    crossbar_pct_under_ncu=90.63,       # ...wavefronts_mem_shared.sum.pct_of_peak_sustained_elapsed
+    duration_ms_under_ncu=121.93,
 )
 FOLD_SOURCES = ("fold_pair.cu", "fold_common.cuh", "periodic_search.cuh", "common.cuh")
 
