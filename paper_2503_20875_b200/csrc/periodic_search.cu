@@ -13,6 +13,7 @@
 #include "fold_common.cuh"
 
 #include <math.h>
+#include <stdlib.h>
 
 #include <algorithm>
 #include <vector>
@@ -180,11 +181,21 @@ int build_periodic_plan(int32_t n_lc, int32_t n_dur, cetra_t0_grid grid, const d
     const size_t row_bytes = static_cast<size_t>(P.stats_pitch) * sizeof(float2);
     const size_t header = kGrpHeaderBytes;
     pl->row_in_smem = row_bytes + header <= static_cast<size_t>(smem_limit);
+    {
+        // test hook: CETRA_FORCE_STREAM=1 sends rows that would fit in shared memory through the streamed kernel, so
+        // that small problems (which the oracle folds in full) exercise it too
+        const char *env = getenv("CETRA_FORCE_STREAM");
+        if (env && env[0] == '1') pl->row_in_smem = false;
+    }
     if (pl->row_in_smem) {
         pl->smem_bytes = row_bytes + header;
     } else {
         // streamed kernel: the ring takes all the shared memory of the SM
         pl->stage_cells = static_cast<int>(((static_cast<size_t>(smem_limit) - kStrHeaderBytes) / (8 * kStrStages)) & ~size_t(1));
+        if (const char *env = getenv("CETRA_STREAM_STAGE_CELLS")) {     // test hook: small stages (block splitting, direct epochs)
+            const int v = atoi(env) & ~1;
+            if (v >= 64 && v < pl->stage_cells) pl->stage_cells = v;
+        }
         pl->smem_bytes = kStrHeaderBytes + static_cast<size_t>(kStrStages) * pl->stage_cells * 8;
     }
     // work units: consecutive periods of one row, one period (per-period kernel) or kGrpT periods (grouped

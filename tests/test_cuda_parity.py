@@ -724,3 +724,101 @@ def test_status_codes_on_device(torch_cuda, cetra):
     before = cetra.cetra_kernel_launch_count()
     cetra.cetra_linear_search(p.times, flux, err, p.durations, p.t0_start, p.t0_stride, p.n_t0, p.template)
     assert cetra.cetra_kernel_launch_count() - before == 3      # preprocess, taps, windowed sums
+
+
+# ------------------------------------------------------------------------------- random geometries
+def _random_light_curve(rng, n, cadence, template):
+    """A small seeded light curve with a few box-ish dips, null points and unequal errors (cetra_synth has the
+    recipes of the BASELINE configs; this one only has to exercise geometry)."""
+    times = 3.0 + np.arange(n) * cadence
+    err = rng.uniform(3e-4, 2e-3, size=n)
+    flux = 1.0 + rng.normal(size=n) * err
+    for _ in range(3):
+        c, w = rng.uniform(times[0], times[-1]), rng.uniform(4, 40) * cadence
+        flux -= 2e-3 * (np.abs(times - c) < w / 2)
+    bad = rng.random(n) < 0.03
+    flux[bad] = np.nan
+    lo = int(rng.integers(0, n - 40))
+    err[lo:lo + int(rng.integers(5, 40))] = np.inf               # a gap of null points
+    return times, flux.astype(np.float32), err.astype(np.float32)
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_linear_search_random_geometries(seed, torch_cuda, cetra, oracle_mod):
+    """The three linear-search paths on random small problems, every cell against the oracle: strides on the sample grid
+    (q = 1..5), rational off-grid strides p/q with random p, q and start (residue classes: p < q, p > q, a single
+    class, starts before the data), and strides that are no small rational multiple (stepped per-cell kernel)."""
+    from cetra_synth import tabulate_template
+    rng = np.random.default_rng(9000 + seed)
+    n = int(rng.integers(300, 2500))
+    cadence = float(rng.choice([20.0, 120.0, 600.0])) / 86400.0
+    tpl = tabulate_template(int(rng.choice([64, 333, 1024])))
+    times, flux, err = _random_light_curve(rng, n, cadence, tpl)
+    durations = np.sort(rng.uniform(2.0, 60.0, size=int(rng.integers(1, 6)))) * cadence
+    fl, er = _dev(torch_cuda, flux), _dev(torch_cuda, err)
+    kinds = ["grid", "rational", "rational", "general"]
+    for kind in kinds:
+        if kind == "grid":
+            stride = int(rng.integers(1, 6)) * cadence
+            start = times[0] + int(rng.integers(-30, 30)) * cadence
+        elif kind == "rational":
+            q = int(rng.integers(1, 24)); p = int(rng.integers(1, 2 * q + 2))
+            stride = cadence * p / q
+            start = times[0] + rng.uniform(-25, 25) * cadence if rng.random() < 0.7 else times[0] - 3 * cadence
+        else:
+            stride = cadence * rng.uniform(0.05, 2.5) * (1.0 + 1.0 / 1009.0)
+            start = times[0] + rng.uniform(-25, 25) * cadence
+        n_t0 = int(min(6000, max(10, (times[-1] - start + 20 * cadence) / stride)))
+        o = oracle_mod.linear_search(times, flux, err, durations, start, stride, n_t0, tpl)
+        r = cetra.cetra_linear_search(times, fl, er, durations, start, stride, n_t0, tpl, want_stats=True)
+        assert_linear_parity(r.depth.cpu().numpy(), r.depth_var.cpu().numpy(), r.dlogL.cpu().numpy(),
+                             o.depth, o.depth_var, o.dlogL, what=f"seed {seed} {kind} stride/c = {stride / cadence:.6f}")
+        st = r.stats[0].cpu().numpy()
+        assert np.all(st[:, n_t0:] == 0) and np.all(st[:, :n_t0, 0][np.isnan(o.depth)] == 0)
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_periodic_search_random_geometries_both_fold_kernels(seed, torch_cuda, cetra, oracle_mod, monkeypatch):
+    """Random small grids and period sets folded by the resident-row kernel and, through the library's test hooks
+    (CETRA_FORCE_STREAM, small CETRA_STREAM_STAGE_CELLS), by the streamed kernel with its epoch blocks split and some
+    windows too wide for a stage: identical records from both, and parity with the oracle on every period."""
+    from cetra_synth import tabulate_template
+    rng = np.random.default_rng(7000 + seed)
+    n = int(rng.integers(800, 3000))
+    cadence = 120.0 / 86400.0
+    tpl = tabulate_template(256)
+    times, flux, err = _random_light_curve(rng, n, cadence, tpl)
+    durations = np.sort(rng.uniform(3.0, 40.0, size=int(rng.integers(2, 5)))) * cadence
+    stride = cadence * float(rng.choice([1.0, 0.5, 0.15, 2.0]))
+    n_t0 = int((times[-1] - times[0]) / stride) + 1
+    span = times[-1] - times[0]
+    kinds = rng.integers(0, 3)
+    if kinds == 0:
+        periods = 1.0 / np.linspace(1.0 / (0.6 * span), 1.0 / (30 * cadence), int(rng.integers(50, 400)))
+    elif kinds == 1:
+        periods = rng.uniform(20 * cadence, 1.5 * span, size=int(rng.integers(30, 200)))      # unsorted, far apart
+    else:
+        periods = np.sort(rng.uniform(40 * cadence, 0.3 * span, size=int(rng.integers(30, 200))))
+    fl, er = _dev(torch_cuda, flux), _dev(torch_cuda, err)
+    lin = cetra.cetra_linear_search(times, fl, er, durations, times[0], stride, n_t0, tpl, want_stats=True)
+    torch_cuda.cuda.synchronize()
+    import oracle as oracle_pkg
+    g64 = oracle_pkg.LinearGrids(*(a.cpu().numpy().astype(np.float64) for a in (lin.depth, lin.depth_var, lin.dlogL)))
+    orc = oracle_mod.periodic_search(g64, times[0], stride, durations, periods)
+    cell = lambda k, j, ph: oracle_mod.periodic_cell(g64, stride, periods[k], j, ph)
+    run = lambda: cetra.peaks_to_numpy(cetra.cetra_periodic_search_stats(lin.stats, n_t0, times[0], stride, durations,
+                                                                         periods))[0]
+    resident = run()
+    assert_periodic_parity(resident, orc, cell, what=f"seed {seed} resident-row fold")
+    monkeypatch.setenv("CETRA_FORCE_STREAM", "1")
+    streamed = run()
+    monkeypatch.setenv("CETRA_STREAM_STAGE_CELLS", str(int(rng.choice([96, 200, 600]))))
+    streamed_small = run()
+    monkeypatch.delenv("CETRA_FORCE_STREAM"); monkeypatch.delenv("CETRA_STREAM_STAGE_CELLS")
+    assert_periodic_parity(streamed, orc, cell, what=f"seed {seed} streamed fold")
+    assert_periodic_parity(streamed_small, orc, cell, what=f"seed {seed} streamed fold, small stages")
+    same = lambda a, b: np.array_equal(a["i_t0"], b["i_t0"]) and np.array_equal(a["j_dur"], b["j_dur"]) and \
+        np.array_equal(a["n_transits"], b["n_transits"])
+    assert same(streamed, streamed_small)
+    # the two kernels add a cell's epochs in different orders: same winners except at FP32 near-ties
+    assert np.mean((resident["i_t0"] == streamed["i_t0"]) & (resident["j_dur"] == streamed["j_dur"])) >= 0.97
