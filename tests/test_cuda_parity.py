@@ -405,6 +405,39 @@ def test_config4_whole_path_sampled(torch_cuda, cetra, oracle_mod):
     assert int(np.nanargmax(pk["lr"])) == int(np.nanargmax(orc.lr))
 
 
+def test_config2_on_the_papers_default_t0_grid(torch_cuda, cetra, oracle_mod):
+    """The TESS-like sector searched as the paper does by default (t0 stride = 1 % of the shortest
+    duration = 18 s = 3/20 of the cadence, I = 131 514 cells, rows of 1 MB): residue-class linear kernel against the
+    oracle on every cell, then the streamed fold on a seeded subset of the 20 000 periods plus windows around the
+    injected period and its aliases; the injected planet must come out at the identical (period, t0, duration)."""
+    p = _problem(2)
+    stride = 0.01 * p.durations[0]
+    t0_start = p.times[0]
+    n_t0 = int((p.times[-1] - p.times[0]) / stride) + 1
+    assert n_t0 == 131514
+    o = oracle_mod.linear_search(p.times, p.flux, p.flux_err, p.durations, t0_start, stride, n_t0, p.template)
+    flux, err = _dev(torch_cuda, p.flux), _dev(torch_cuda, p.flux_err)
+    lin = cetra.cetra_linear_search(p.times, flux, err, p.durations, t0_start, stride, n_t0, p.template, want_stats=True)
+    worst = assert_linear_parity(lin.depth.cpu().numpy(), lin.depth_var.cpu().numpy(), lin.dlogL.cpu().numpy(),
+                                 o.depth, o.depth_var, o.dlogL, what="config 2, default t0 grid")
+    inj = [i["period"] for i in p.injections]
+    sel = period_subset(p.periods, inj, 60, seed=22, half_width=15)
+    periods = p.periods[sel]
+    pk = cetra.peaks_to_numpy(cetra.cetra_periodic_search_stats(lin.stats, n_t0, t0_start, stride, p.durations,
+                                                                periods))[0]
+    orc = oracle_mod.periodic_search(o, t0_start, stride, p.durations, periods)
+    must = [int(np.argmin(np.abs(periods - inj[0])))]
+    res = assert_periodic_parity(pk, orc, lambda k, j, ph: oracle_mod.periodic_cell(o, stride, periods[k], j, ph),
+                                 what="config 2, default t0 grid, streamed fold", must_match=must)
+    print("default t0 grid:", worst, res, "periods", periods.shape[0])
+    kb = int(np.nanargmax(pk["lr"]))
+    assert kb == int(np.nanargmax(orc.lr)) and abs(periods[kb] - inj[0]) <= 0.01 * inj[0]
+    # the batched entry point runs the same two kernels: identical records
+    pb = cetra.peaks_to_numpy(cetra.cetra_search_batched(p.times, flux[None], err[None], p.durations, t0_start, stride,
+                                                         n_t0, p.template, periods))[0]
+    assert np.array_equal(pb.view(np.uint8), pk.view(np.uint8))
+
+
 # ------------------------------------------------------------------------------------------ batched
 def test_batched_equals_single_and_host_variant(torch_cuda, cetra, oracle_mod):
     """Survey batch (config 5 recipe, 7 light curves, chunks of 3 -> ragged last chunk): the batched call,
