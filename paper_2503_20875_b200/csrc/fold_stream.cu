@@ -57,7 +57,7 @@ static_assert(kStrUnitPeriods == kStrWarps * kGrpT && kStrUnitPeriods % 2 == 0, 
 static_assert(kStrUnitPeriods <= 64, "the producer warp holds a unit's periods two per lane");
 
 enum : int {
-    kFirstOfPass = 1,      // reset the accumulators
+    kFirstOfPass = 1,      // the block holds epoch 0 of a pass
     kLastOfPass = 2,       // combine + per-lane argmax (P3, P4) after this block
     kFirstOfUnit = 4,      // decode the unit, load and sort the warp's periods
     kLastOfUnit = 8,       // publish the warp's two keys after this block
@@ -92,7 +92,8 @@ struct StreamSmem {
     uint64_t empty[kStrStages];
     StageDesc desc[kStrStages];
 };
-constexpr int kStrWordsOffset = static_cast<int>((sizeof(StreamSmem) + 1023) / 1024 * 1024);                    // per-warp epoch words: (kStrBlock + 1) x 16 bytes each
+// per-warp epoch words behind the barriers and descriptors: (kStrBlock + 1) x 16 bytes each
+constexpr int kStrWordsOffset = static_cast<int>((sizeof(StreamSmem) + 1023) / 1024 * 1024);
 constexpr int kStrWordsPitch = (kStrBlock + 1) * 16 + 16;
 static_assert(sizeof(StreamSmem) <= kStrWordsOffset, "header");
 static_assert(kStrWordsOffset + (kStrThreads / 32 - 1) * kStrWordsPitch <= kStrHeaderBytes, "header");
