@@ -170,8 +170,9 @@ def oracle_sample(p, flux, flux_err, budget_s: float, threads: int = 0):
     import oracle
     oracle.build()
     all_threads = oracle.get_threads()
-    if threads > 0:
-        oracle.set_threads(threads)
+    # all the cores this process may use, stated explicitly: torchrun exports OMP_NUM_THREADS=1 to its ranks, which
+    # would silently turn the N > 1 reference arm into a one-thread run
+    oracle.set_threads(threads if threads > 0 else len(os.sched_getaffinity(0)))
     try:
         return _oracle_sample(oracle, p, flux, flux_err, budget_s)
     finally:
