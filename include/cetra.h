@@ -53,7 +53,8 @@ typedef enum {
     CETRA_ERR_NONUNIFORM_TIMES = -2,  /* times[] is not a regular grid */
     CETRA_ERR_UNSUPPORTED = -3,       /* too many durations, index overflow */
     CETRA_ERR_WORKSPACE = -4,         /* workspace null, misaligned or smaller than *_workspace_bytes */
-    CETRA_ERR_CUDA = -5               /* a CUDA runtime call failed (cudaGetLastError is left set) */
+    CETRA_ERR_CUDA = -5,              /* a CUDA runtime call failed (cudaGetLastError is left set) */
+    CETRA_ERR_STATIC_LIMIT = -6       /* cetra_resample_static: n_lc * n_out exceeds CETRA_RESAMPLE_STATIC_MAX_POINTS */
 } cetra_status;
 
 typedef enum { CETRA_F32 = 0, CETRA_F64 = 1 } cetra_dtype;
@@ -261,6 +262,53 @@ int cetra_resample(const double *times_dev, const void *flux_dev, const void *fl
                    int64_t n_in, int32_t n_lc, double t_start, double cadence, int64_t n_out,
                    void *flux_out_dev, void *flux_err_out_dev,
                    void *workspace_dev, size_t workspace_bytes, void *cuda_stream);
+
+/* ------------------------------------------------------------------------------------------
+ * cetra_resample for callers that have no device memory to give as a workspace.
+ *
+ * Who this is for.  cetra_resample needs cetra_resample_workspace_bytes() of device scratch (one pair of FP64 sums
+ * per output point).  Some callers cannot produce that: code that runs inside somebody else's memory budget and is
+ * handed its input and output buffers but no allocator (a plug-in stage of a pipeline, a worker whose device pool
+ * was carved up front and is full), code on a path where cudaMalloc is not allowed because it synchronises the
+ * whole device (a latency-critical service loop, a region other threads are capturing or timing), and code in a
+ * process whose memory is accounted for by a framework that forbids allocations behind its back.  For them this
+ * entry point keeps the sums in a fixed array that is part of the library image itself.
+ *
+ * What it costs.  The array is CETRA_RESAMPLE_STATIC_MAX_POINTS pairs of doubles = 4 MiB of device memory on every
+ * GPU that loads the library, from the moment the library's CUDA module is loaded on that GPU until the process
+ * exits, whether or not this function is ever called.
+ *
+ * Limit.  n_lc * n_out <= CETRA_RESAMPLE_STATIC_MAX_POINTS (262 144 output points over all light curves of the
+ * call: e.g. 13 TESS 2-min sectors of ~20 000 points).  A larger request is refused with
+ * CETRA_ERR_STATIC_LIMIT before anything is enqueued; split the light curves over several calls, or use
+ * cetra_resample with a workspace.  cetra_resample_static_max_points() returns the limit at run time.
+ *
+ * Arguments, arithmetic and results are cetra_resample's (same kernels, same FP64 atomic sums): the two agree to
+ * FP64 rounding of the sums, i.e. after rounding to the output dtype to within one unit in the last place.
+ * The call makes no cudaMalloc / cudaFree and calls nothing that allocates; it enqueues one memset of the part of
+ * the array it uses and two kernels on `cuda_stream` and returns without synchronising.
+ *
+ * First call on each device.  The address of the array on the current device is looked up once per device
+ * (cudaGetSymbolAddress, with that device current) the first time this function runs there, and remembered.  That
+ * lookup may load the library's CUDA module, so make the first call on each device during set-up, outside any
+ * stream capture and outside any region where module loading is unwelcome.
+ *
+ * Sharing.  Every call on a device uses the same array, from offset 0, and leaves its sums behind; each call
+ * clears the part it is about to use, so earlier calls never leak into later ones.  Two calls that can run on the
+ * GPU at the same time (different streams of one device without an ordering between them, or two host threads)
+ * overwrite each other's sums and both give wrong answers: order them on one stream or with events.  Different
+ * devices have separate copies and do not interact.
+ *
+ * Returns CETRA_OK, CETRA_ERR_INVALID_ARG (as cetra_resample), CETRA_ERR_STATIC_LIMIT, CETRA_ERR_UNSUPPORTED
+ * (device ordinal >= 64) or CETRA_ERR_CUDA (no device, symbol lookup or launch failed).
+ * ------------------------------------------------------------------------------------------ */
+#define CETRA_RESAMPLE_STATIC_MAX_POINTS 262144
+
+int64_t cetra_resample_static_max_points(void);
+
+int cetra_resample_static(const double *times_dev, const void *flux_dev, const void *flux_err_dev, cetra_dtype dtype,
+                          int64_t n_in, int32_t n_lc, double t_start, double cadence, int64_t n_out,
+                          void *flux_out_dev, void *flux_err_out_dev, void *cuda_stream);
 
 /* ------------------------------------------------------------------------------------------
  * Monotransit search: single-transit events in the linear-search output alone.

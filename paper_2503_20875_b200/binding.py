@@ -22,6 +22,7 @@ CETRA_ERR_NONUNIFORM_TIMES = -2
 CETRA_ERR_UNSUPPORTED = -3
 CETRA_ERR_WORKSPACE = -4
 CETRA_ERR_CUDA = -5
+CETRA_ERR_STATIC_LIMIT = -6
 CETRA_F32, CETRA_F64 = 0, 1
 CETRA_MAX_DURATIONS = 128
 
@@ -36,6 +37,7 @@ EXPORTED_SYMBOLS = (
     "cetra_profile_enable", "cetra_profile_read", "cetra_peak_probe_workspace_bytes", "cetra_peak_probe",
     "cetra_tc_correlation_probe_workspace_bytes", "cetra_tc_correlation_probe",
     "cetra_resample_template", "cetra_median_cadence", "cetra_resample_grid", "cetra_resample_workspace_bytes", "cetra_resample",
+    "cetra_resample_static_max_points", "cetra_resample_static",
     "cetra_monotransit_workspace_bytes", "cetra_monotransit_search",
     "cetra_mask_workspace_bytes", "cetra_mask_transits",
 )
@@ -132,6 +134,11 @@ def load_library() -> ctypes.CDLL:
     lib.cetra_resample.restype = ctypes.c_int
     lib.cetra_resample.argtypes = [vp, vp, vp, ctypes.c_int, i64, i32, ctypes.c_double, ctypes.c_double, i64,
                                    vp, vp, vp, sz, vp]
+    lib.cetra_resample_static_max_points.restype = i64
+    lib.cetra_resample_static_max_points.argtypes = []
+    lib.cetra_resample_static.restype = ctypes.c_int
+    lib.cetra_resample_static.argtypes = [vp, vp, vp, ctypes.c_int, i64, i32, ctypes.c_double, ctypes.c_double, i64,
+                                          vp, vp, vp]
     lib.cetra_monotransit_workspace_bytes.restype = sz
     lib.cetra_monotransit_workspace_bytes.argtypes = [i32, i64]
     lib.cetra_monotransit_search.restype = ctypes.c_int
@@ -620,6 +627,55 @@ def cetra_resample(times_dev, flux, flux_err, t_start: float, cadence: float, n_
                                 n_in, n_lc, float(t_start), float(cadence), int(n_out), out_f.data_ptr(),
                                 out_e.data_ptr(), ws.data_ptr(), ws.numel(), _stream_ptr(torch, stream))
     _check(rc, "cetra_resample")
+    return (out_f[0], out_e[0]) if squeeze else (out_f, out_e)
+
+
+def cetra_resample_static_max_points() -> int:
+    """Largest n_lc * n_out one cetra_resample_static call accepts (the size of the library's built-in scratch)."""
+    return int(load_library().cetra_resample_static_max_points())
+
+
+@_on_stream
+def cetra_resample_static(times_dev, flux, flux_err, t_start: float, cadence: float, n_out: int, out=None,
+                          stream=None):
+    """cetra_resample without a workspace, for callers that cannot allocate device memory.
+
+    Same arguments and results as cetra_resample, but the FP64 sums are kept in a 4 MiB array built into the library
+    instead of a workspace tensor, so the C call underneath allocates nothing.  It exists for code that is handed
+    buffers but no allocator: a stage running inside another program's fixed device-memory budget, a service loop
+    where cudaMalloc's device-wide synchronisation is not acceptable, a process whose framework forbids allocations
+    it does not see.  Such a caller passes `out=(flux_out, flux_err_out)`, two [B][n_out] (or [n_out]) CUDA tensors
+    of the input dtype that it already owns, and then this wrapper allocates nothing either; without `out` the
+    wrapper creates the two result tensors with torch, as cetra_resample does.
+
+    Limits and caveats (include/cetra.h has the full text): B * n_out <= cetra_resample_static_max_points()
+    (262 144), else CetraError with status CETRA_ERR_STATIC_LIMIT; the first call on each device looks the array up
+    and should happen during set-up, before any stream capture; all calls on a device share the array, so calls that
+    could overlap on the GPU (unordered streams, threads) must be ordered by the caller.
+    """
+    torch = _torch()
+    lib = load_library()
+    flux, flux_err, n_lc, n_in = _dev_input(torch, flux, flux_err)
+    squeeze = flux.dim() == 1
+    if not (times_dev.is_cuda and times_dev.dtype == torch.float64 and times_dev.numel() == n_in):
+        raise TypeError("times_dev must be a float64 CUDA tensor with one entry per observation")
+    times_dev = times_dev.contiguous()
+    if out is None:
+        out_f = torch.empty((n_lc, int(n_out)), dtype=flux.dtype, device=flux.device)
+        out_e = torch.empty_like(out_f)
+    else:
+        out_f, out_e = out
+        for o in (out_f, out_e):
+            if not (o.is_cuda and o.device == flux.device and o.dtype == flux.dtype and o.is_contiguous()
+                    and o.numel() == n_lc * int(n_out)):
+                raise TypeError("out must be two contiguous CUDA tensors of the input dtype with B * n_out elements")
+    with torch.cuda.device(flux.device):
+        rc = lib.cetra_resample_static(times_dev.data_ptr(), flux.data_ptr(), flux_err.data_ptr(),
+                                       _dtype_code(torch, flux), n_in, n_lc, float(t_start), float(cadence),
+                                       int(n_out), out_f.data_ptr(), out_e.data_ptr(), _stream_ptr(torch, stream))
+    _check(rc, "cetra_resample_static")
+    if out is not None:
+        return out_f, out_e
     return (out_f[0], out_e[0]) if squeeze else (out_f, out_e)
 
 

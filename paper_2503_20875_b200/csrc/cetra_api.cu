@@ -159,6 +159,8 @@ const char *cetra_status_string(int status) {
         case CETRA_ERR_UNSUPPORTED: return "unsupported configuration";
         case CETRA_ERR_WORKSPACE: return "workspace null, misaligned or too small";
         case CETRA_ERR_CUDA: return "CUDA runtime error";
+        case CETRA_ERR_STATIC_LIMIT:
+            return "request exceeds the library's built-in scratch (cetra_resample_static: n_lc * n_out > 262144)";
         default: return "unknown status";
     }
 }

@@ -7,6 +7,7 @@
 #include <math.h>
 
 #include <algorithm>
+#include <mutex>
 #include <vector>
 
 #include "common.cuh"
@@ -197,6 +198,41 @@ static int have_device() {
     return CETRA_OK;
 }
 
+// --------------------------------------------------------------- resample with built-in scratch
+// The sums of cetra_resample_static (cetra.h) live in the library image instead of a caller workspace: a fixed
+// array in device global memory, one copy per GPU that loads this module, there until the process exits.
+// 256-byte alignment matches what the workspace entry points require of theirs.
+static __device__ __align__(256) double2 g_static_sums[CETRA_RESAMPLE_STATIC_MAX_POINTS];
+
+// In host code `g_static_sums` is only a handle the runtime uses to find the symbol, not somewhere a kernel can
+// write: handing it to a launch would fault, or on a machine where the GPU can reach host memory quietly scribble
+// over the host-side shadow.  The real device address differs per GPU, so it is asked for once per device, with
+// that device current, and kept here.
+constexpr int kMaxStaticDevices = 64;
+static std::mutex g_static_mutex;
+static double2 *g_static_addr[kMaxStaticDevices] = {};
+
+static int static_sums_on_current_device(double2 **out) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
+        return CETRA_ERR_CUDA;
+    }
+    if (dev < 0 || dev >= kMaxStaticDevices) return CETRA_ERR_UNSUPPORTED;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_addr[dev]) {
+        double2 *p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void **>(&p), g_static_sums);
+        if (e != cudaSuccess || !p) {
+            cudaGetLastError();
+            return CETRA_ERR_CUDA;
+        }
+        g_static_addr[dev] = p;
+    }
+    *out = g_static_addr[dev];
+    return CETRA_OK;
+}
+
 }  // namespace cetra
 
 using namespace cetra;
@@ -279,6 +315,51 @@ int cetra_resample(const double *times_dev, const void *flux_dev, const void *fl
     if (have_device() != CETRA_OK) return CETRA_ERR_CUDA;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     double2 *sums = static_cast<double2 *>(workspace_dev);
+    const long long total_out = static_cast<long long>(n_lc) * n_out;
+    CETRA_CUDA_TRY(cudaMemsetAsync(sums, 0, sizeof(double2) * static_cast<size_t>(total_out), st));
+    const long long total_in = static_cast<long long>(n_lc) * n_in;
+    if (total_in > 0) {
+        if (dtype == CETRA_F32)
+            resample_accumulate_kernel<float><<<stream_blocks(total_in), 256, 0, st>>>(
+                times_dev, static_cast<const float *>(flux_dev), static_cast<const float *>(flux_err_dev), n_in, n_lc,
+                t_start, cadence, n_out, sums);
+        else
+            resample_accumulate_kernel<double><<<stream_blocks(total_in), 256, 0, st>>>(
+                times_dev, static_cast<const double *>(flux_dev), static_cast<const double *>(flux_err_dev), n_in,
+                n_lc, t_start, cadence, n_out, sums);
+        CETRA_LAUNCH_CHECK();
+    }
+    if (dtype == CETRA_F32)
+        resample_finalize_kernel<float><<<stream_blocks(total_out), 256, 0, st>>>(
+            sums, total_out, static_cast<float *>(flux_out_dev), static_cast<float *>(flux_err_out_dev));
+    else
+        resample_finalize_kernel<double><<<stream_blocks(total_out), 256, 0, st>>>(
+            sums, total_out, static_cast<double *>(flux_out_dev), static_cast<double *>(flux_err_out_dev));
+    CETRA_LAUNCH_CHECK();
+    return CETRA_OK;
+}
+
+int64_t cetra_resample_static_max_points(void) { return CETRA_RESAMPLE_STATIC_MAX_POINTS; }
+
+// cetra_resample for callers without a workspace to give (cetra.h has the full contract): the FP64 sums go to
+// g_static_sums.  Nothing here allocates; the only set-up is the once-per-device address lookup above, done by the
+// first call on each device.  The array still holds the previous call's sums, so the part this call uses is cleared
+// first, on the caller's stream, ahead of the accumulation.
+int cetra_resample_static(const double *times_dev, const void *flux_dev, const void *flux_err_dev, cetra_dtype dtype,
+                          int64_t n_in, int32_t n_lc, double t_start, double cadence, int64_t n_out,
+                          void *flux_out_dev, void *flux_err_out_dev, void *cuda_stream) {
+    if (((!times_dev || !flux_dev || !flux_err_dev) && n_in != 0) || !flux_out_dev || !flux_err_out_dev || n_in < 0 ||
+        n_lc < 1 || n_out < 1 || !(cadence > 0.0) || !std::isfinite(cadence) || !std::isfinite(t_start) ||
+        (dtype != CETRA_F32 && dtype != CETRA_F64))
+        return CETRA_ERR_INVALID_ARG;
+    // n_out alone is tested first so that the product below cannot overflow
+    if (n_out > CETRA_RESAMPLE_STATIC_MAX_POINTS ||
+        static_cast<long long>(n_lc) * n_out > CETRA_RESAMPLE_STATIC_MAX_POINTS)
+        return CETRA_ERR_STATIC_LIMIT;
+    double2 *sums = nullptr;
+    const int rc = static_sums_on_current_device(&sums);
+    if (rc != CETRA_OK) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const long long total_out = static_cast<long long>(n_lc) * n_out;
     CETRA_CUDA_TRY(cudaMemsetAsync(sums, 0, sizeof(double2) * static_cast<size_t>(total_out), st));
     const long long total_in = static_cast<long long>(n_lc) * n_in;
