@@ -74,3 +74,18 @@ def period_subset(periods, injected, n_random, seed, half_width=60):
             k0 = int(np.argmin(np.abs(periods - target)))
             pick.update(range(max(0, k0 - half_width), min(K, k0 + half_width + 1)))
     return np.array(sorted(pick), dtype=np.int64)
+
+
+def nearest_template_sample(x, M):
+    """Index of the tabulated template sample nearest to position x in [0, 1] ("the nearest model point
+    is selected"), straight from the definition: the template's M samples sit at m / (M - 1), m = 0 .. M-1 (first to
+    last contact), and the nearest one is found by comparing distances.  No rounding expression is involved, so a test
+    that takes its indices from here does not repeat the oracle's (or the kernels') arithmetic.  Also returns the
+    margin by which the nearest sample wins over the runner-up, so callers can keep clear of exact half-steps, where
+    "nearest" has two answers."""
+    x = np.atleast_1d(np.asarray(x, dtype=np.float64))
+    pos = np.arange(M, dtype=np.float64) / (M - 1.0)
+    dist = np.abs(x[:, None] - pos[None, :])
+    order = np.argsort(dist, axis=1, kind="stable")
+    rows = np.arange(x.shape[0])
+    return order[:, 0], dist[rows, order[:, 1]] - dist[rows, order[:, 0]]

@@ -3,6 +3,8 @@ PAPER.md:87, which does not sit on the sample grid).  CPU only."""
 import numpy as np
 import pytest
 
+from parity_util import nearest_template_sample
+
 
 def _lc(n, c, sigma, seed):
     rng = np.random.default_rng(seed)
@@ -50,7 +52,11 @@ def test_off_grid_cell_is_the_weighted_least_squares_fit(oracle_mod):
             x = (t - ti) / D + 0.5
             win = (x >= 0) & (x <= 1) & np.isfinite(f)
             assert np.min(np.abs(x[np.isfinite(f)] - 0.0)) > 1e-9 and np.min(np.abs(x[np.isfinite(f)] - 1.0)) > 1e-9
-            m = tpl[np.floor(x[win] * (len(tpl) - 1) + 0.5).astype(int)]
+            # the template sample of every observation from the definition (distances to the tabulated positions),
+            # not from the oracle's rounding expression
+            idx, margin = nearest_template_sample(x[win], len(tpl))
+            assert margin.min() > 1e-9
+            m = tpl[idx]
             sw = 1.0 / e[win]
             sol, *_ = np.linalg.lstsq((sw * m)[:, None], sw * (1.0 - f[win]), rcond=None)
             assert g.depth[j, i] == pytest.approx(sol[0], rel=1e-9)
@@ -91,7 +97,9 @@ def test_off_grid_noiseless_injection_recovered_exactly(oracle_mod):
     x = (np.arange(n) * c - ti) / durations[j_star] + 0.5
     ins = (x >= 0) & (x <= 1)
     m = np.zeros(n)
-    m[ins] = tpl[np.floor(x[ins] * 1023 + 0.5).astype(int)]
+    idx, margin = nearest_template_sample(x[ins], 1024)
+    assert margin.min() > 1e-9
+    m[ins] = tpl[idx]
     f = 1.0 - depth * m
     e = np.full(n, 3e-4)
     g = oracle_mod.linear_search(t, f, e, durations, t0_start, s, 3000, tpl)
