@@ -44,6 +44,8 @@ UNIT = "light curves/s"
 L2_FLUSH_BYTES = 512 << 20
 N_SM, FP32_LANES = 148, 128          # B200: SMs, FP32 FMA lanes per SM (B200_PROFILING.md unit counts)
 SMEM_BYTES_PER_CLK = 128             # shared-memory crossbar bytes/clk/SM (B300_MICROARCH.md, LDS/STS)
+# nominal per-clock per-SM rates of the probed instructions: 128 lanes x 2 flop (FFMA2), x 1 flop (FADD2), crossbar bytes
+PROBE_NOMINAL = dict(ffma2=2.0 * FP32_LANES, fadd2=1.0 * FP32_LANES, lds64=float(SMEM_BYTES_PER_CLK))
 # Counters of ONE fold_pair_argmax_kernel launch over the 64-curve chunk of this workload, from the `ncu --set full`
 # capture summarised in `profile` (command inside).  They are properties of the launch (the kernel's loads do not
 # depend on timing), valid for the kernel sources whose hash is `src_sha256`: bench.py hashes the sources it runs
@@ -223,9 +225,13 @@ def run_reference(args, rank: int):
     wall = time.perf_counter() - t0
     value = len(vals) / sum(1.0 / v for v in vals)
     line = dict(metric=METRIC, value=value, unit=UNIT, impl="reference", n_gpus=args.gpus, steps=args.steps,
-                warmup=args.warmup, ms_per_step=1e3 * wall / max(args.steps, 1), higher_is_better=True,
+                warmup=args.warmup, ms_per_step=1e3 / value, higher_is_better=True,
                 scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
-                config=workload_config(p, args.n_lc), notes="oracle on host cores; each step = " + sample,
+                config=workload_config(p, args.n_lc),
+                notes="oracle on host cores; each step = " + sample + "; ms_per_step is the time `value` counts (one "
+                      "light curve, periodic part scaled to all periods); ms_wall_per_step also holds the passes that "
+                      "size the subset and ms_timed_per_step only the linear search and the timed subset",
+                ms_wall_per_step=1e3 * wall / max(args.steps, 1), ms_timed_per_step=1e3 * spent / max(args.steps, 1),
                 cpu_baseline=dict(value=value, unit=UNIT, cores=cores, kind="oracle", sample=sample),
                 e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
                 gpu_launches=0)
@@ -317,7 +323,13 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
     for name, kind in (("ffma2", cetra.CETRA_PROBE_FFMA2), ("fadd2", cetra.CETRA_PROBE_FADD2),
                        ("lds64", cetra.CETRA_PROBE_LDS64)):
         per_clk, per_s = cetra.cetra_peak_probe(kind)
-        probes[name] = dict(per_clk_per_sm=per_clk, per_second=per_s, unit="B" if name == "lds64" else "flop")
+        probes[name] = dict(per_clk_per_sm=per_clk, per_second=per_s, unit="B" if name == "lds64" else "flop",
+                            nominal_per_clk_per_sm=PROBE_NOMINAL[name])
+        # a probe above the unit's physical rate is a broken probe (round 2: ptxas merged the LDS probe's repeated
+        # addresses and it read 3.0 x the crossbar), and a roofline beside it would be unexplained: refuse to print one
+        if per_clk > 1.05 * PROBE_NOMINAL[name]:
+            raise SystemExit(f"bench.py: cetra_peak_probe({name}) measured {per_clk:.1f} per clock per SM, above the "
+                             f"unit's nominal {PROBE_NOMINAL[name]}: the probe is not measuring what it claims")
     with ClockSampler(local_rank) as clocks:
         ms_dev, launches, prof, wall_dev = timed(step_device, args.steps, profile=True)
     ms_e2e, _, _, wall_e2e = timed(step_host, args.steps, profile=False)
@@ -338,8 +350,10 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
     # -- dominant kernel: the periodic fold.  Physical level: shared-memory crossbar (LDS bytes / probe rate).
     sha = fold_sources_sha256()
     stale = sha != NCU_FOLD["src_sha256"]
-    lds_bytes = 128.0 * NCU_FOLD["lds_wavefronts"] * lc_per_launch / NCU_FOLD["n_lc"]
-    lds_gbs = lds_bytes / (fold_ms * 1e-3) / 1e9
+    # the wavefront count belongs to the sources it was captured from: with edited fold sources there is no
+    # crossbar figure (achieved / frac / lds_bytes_per_launch are null and `ncu.stale` says why), only the yardstick
+    lds_bytes = None if stale else 128.0 * NCU_FOLD["lds_wavefronts"] * lc_per_launch / NCU_FOLD["n_lc"]
+    lds_gbs = None if stale else lds_bytes / (fold_ms * 1e-3) / 1e9
     smem_peak_gbs = N_SM * SMEM_BYTES_PER_CLK * peaks["sm_max_mhz"] * 1e6 / 1e9
     # north_star's yardstick: 8 B gathered and 2 FADD per (period, duration, t0 cell) against the HBM copy peak
     alg_bytes = 8.0 * wc["gathers"] * lc_per_launch
@@ -358,7 +372,7 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
         clocks=clocks.summary(),
         roofline=dict(
             bound="smem", kernel="fold_pair_argmax_kernel", achieved=lds_gbs, peak=smem_peak_gbs, unit="GB/s",
-            frac=lds_gbs / smem_peak_gbs,
+            frac=None if stale else lds_gbs / smem_peak_gbs,
             traffic=None if stale else NCU_FOLD["dram_bytes"] * lc_per_launch / NCU_FOLD["n_lc"],
             derivation="achieved = shared-memory bytes the kernel's loads move per launch (ncu LDS wavefronts of "
                        "this workload x 128 B, scaled to the curves per launch) / its average event-timed "
@@ -370,7 +384,7 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
             ncu=dict(NCU_FOLD, stale=stale, src_sha256_now=sha),
             algorithmic=dict(bytes_per_launch=alg_bytes, gbs=alg_gbs, hbm_peak_gbs=peaks["hbm_gbs"],
                              over_hbm_peak=alg_gbs / peaks["hbm_gbs"], hbm_peak_source=peaks["source"],
-                             loads_per_cell=lds_bytes / alg_bytes,
+                             loads_per_cell=None if stale else lds_bytes / alg_bytes,
                              note="north_star's yardstick (8 B per (period, duration, t0 cell) / HBM copy peak); "
                                   "a ratio above 1 is reuse, not a roofline fraction: a row is read from HBM a "
                                   "handful of times per launch and gathered from shared memory 20 000 times")),
@@ -513,10 +527,11 @@ def run_configs(args):
                                                                       p.periods), max(1, min(reps, 3)))
             og_bytes = 8.0 * wc["pairs"] * n_t0
             print(json.dumps(dict(workload="configs[1] on the paper's default t0 grid (stride = 1 % of the shortest "
-                                           "duration, off the sample grid): linear_general_kernel, then the "
-                                           "large-row fold kernel (1.05 MB rows)",
+                                           "duration = 18 s = 3/20 of the cadence, off the sample grid): "
+                                           "linear_search_kernel on residue classes of cells, then the streamed "
+                                           "fold kernel (1.05 MB rows)",
                                   n_t0=n_t0, linear_ms=og_ms, template_evals_per_s=evals / (og_ms * 1e-3),
-                                  bound="fp64 index arithmetic (one IEEE division per template evaluation)",
+                                  bound="alu (FP32 FMA; the polyphase branches of a class pad their taps)",
                                   periodic_ms=ogp_ms, fold_algorithmic_gbs=og_bytes / (ogp_ms * 1e-3) / 1e9,
                                   light_curves_per_s=1e3 / (og_ms + ogp_ms))), flush=True)
     # setup kernels: resampling 64 irregular light curves of 200 000 observations (HBM-bound streaming)

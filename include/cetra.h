@@ -27,10 +27,14 @@
  *  - The t0 grid is t_i = t0_start + i*t0_stride, i < n_t0, any start and any stride > 0.
  *    When every t0 cell lies on a sample (to 1e-6 cadence at the last cell: |a - round a| + |b - round b| (n_t0-1)
  *    <= 1e-6 with a = (t0_start - times[0])/c, b = t0_stride/c, b >= 1)
- *    the nearest-neighbour template position comes from the integer sample offset (R3) and the fast
- *    tabulated-tap kernel runs; otherwise (e.g. the paper's default stride, 1 % of the shortest duration)
- *    it comes from the time difference x = (n*c - (t_i - times[0]))/D + 1/2 in FP64 (R25) and a per-cell
- *    kernel runs.  t0_start may lie before times[0] or t_i after times[n-1]: windows are clipped to the
+ *    the nearest-neighbour template position comes from the integer sample offset (R3) and the
+ *    tabulated-tap kernel runs; otherwise it comes from the time difference
+ *    x = (n*c - (t_i - times[0]))/D + 1/2 in FP64 (R25).  Off the sample grid a stride that is a small rational
+ *    multiple of the cadence (the paper's default, 1 % of the shortest duration: 18 s on 2-min data = 3/20) is
+ *    split into residue classes of cells, each an on-grid problem for the same tabulated-tap kernel with its own
+ *    tap tables; any other stride takes a per-cell kernel that steps the position in fixed point.  Both evaluate
+ *    the exact R25 sequence only where a position lies within a proven rounding bound of a decision point
+ *    (cetra_exact_eval_count), so the result is the definition's on every path.  t0_start may lie before times[0] or t_i after times[n-1]: windows are clipped to the
  *    data (R9), which is the paper's null padding expressed through the grid.
  *  - Grids are stored [n_dur][n_t0], t0 contiguous, float32.  Cells whose window holds no
  *    observation are NaN in all three grids.
@@ -105,6 +109,8 @@ int cetra_device_info(int32_t *n_sm, int32_t *smem_per_block_optin);
  *  stats_dev      optional output (may be NULL): the sufficient statistics (S_wmm, S_wmf) as float2,
  *                 [n_lc][n_dur][cetra_stats_pitch(n_t0)], zero in null cells and in the row padding;
  *                 this is the form cetra_periodic_search_stats consumes.
+ *  Limits: n_lc <= 65 535 per call (light curves are one dimension of the launch grid; more return
+ *  CETRA_ERR_UNSUPPORTED: call once per slice of curves, or use cetra_search_batched, which slices by itself).
  * ------------------------------------------------------------------------------------------ */
 size_t cetra_linear_workspace_bytes(const double *times_host, int64_t n, int32_t n_lc,
                                     const double *durations_host, int32_t n_dur,
@@ -169,7 +175,8 @@ int cetra_periodic_search_stats(const float *stats_dev, int32_t n_lc, int32_t n_
 /* ------------------------------------------------------------------------------------------
  * Batched search: n_lc light curves sharing one timestamp array, linear search then
  * periodic search per chunk of light curves; the per-curve grids live only in the workspace.
- * Arguments as above.  `lc_chunk` light curves are resident at a time (0 = library default).
+ * Arguments as above.  `lc_chunk` light curves are resident at a time (0 = library default; a larger request is
+ * clamped to 65 535, the most one linear-search launch takes).  n_lc itself is not limited.
  * ------------------------------------------------------------------------------------------ */
 size_t cetra_search_batched_workspace_bytes(const double *times_host, int64_t n, int32_t n_lc, int32_t lc_chunk,
                                             const double *durations_host, int32_t n_dur, cetra_t0_grid grid,
@@ -364,6 +371,16 @@ int cetra_mask_transits(const double *times_dev, void *flux_dev, cetra_dtype dty
 
 /* Number of kernel launches the library has enqueued since the process started (diagnostic). */
 int64_t cetra_kernel_launch_count(void);
+
+/* Test hook, not a tuning knob: overrides the periodic search's choice of fold kernel for every later call in
+ * this process, so that the parity tests can send small problems (which the oracle folds in full) through the kernel
+ * that normally serves only rows too large for shared memory.  force_stream != 0: rows that fit in shared memory are
+ * streamed anyway; stage_cells >= 64: the streamed kernel's stages hold that many cells instead of a full share of
+ * shared memory (epoch blocks split, wide windows gathered directly).  (0, 0) restores the library's own plan, which
+ * is the only one production code should run: the overridden plans give the same records, more slowly.
+ * The library reads no environment variable; this call is the only way to change the plan.  Not thread-safe with
+ * respect to searches running concurrently on other host threads. */
+void cetra_test_fold_override(int32_t force_stream, int32_t stage_cells);
 
 /* Diagnostics for bench.py's roofline line.  While enabled, the library brackets every launch of its two
  * hot kernels (the windowed-sum linear-search kernel and the fold-gather-argmax periodic-search kernel)

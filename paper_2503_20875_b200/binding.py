@@ -37,7 +37,7 @@ EXPORTED_SYMBOLS = (
     "cetra_profile_enable", "cetra_profile_read", "cetra_peak_probe_workspace_bytes", "cetra_peak_probe",
     "cetra_tc_correlation_probe_workspace_bytes", "cetra_tc_correlation_probe",
     "cetra_resample_template", "cetra_median_cadence", "cetra_resample_grid", "cetra_resample_workspace_bytes", "cetra_resample",
-    "cetra_resample_static_max_points", "cetra_resample_static",
+    "cetra_resample_static_max_points", "cetra_resample_static", "cetra_test_fold_override",
     "cetra_monotransit_workspace_bytes", "cetra_monotransit_search",
     "cetra_mask_workspace_bytes", "cetra_mask_transits",
 )
@@ -148,6 +148,8 @@ def load_library() -> ctypes.CDLL:
     lib.cetra_mask_workspace_bytes.argtypes = [i32]
     lib.cetra_mask_transits.restype = ctypes.c_int
     lib.cetra_mask_transits.argtypes = [vp, vp, ctypes.c_int, i64, i32, dp, dp, dp, ctypes.c_double, vp, vp, sz, vp]
+    lib.cetra_test_fold_override.restype = None
+    lib.cetra_test_fold_override.argtypes = [i32, i32]
     lib.cetra_profile_enable.restype = ctypes.c_int
     lib.cetra_profile_enable.argtypes = [i32]
     lib.cetra_profile_read.restype = ctypes.c_int
@@ -322,6 +324,12 @@ def cetra_tc_correlation_probe(n_out: int, n_taps: int, split: bool = True, reps
                                           ctypes.byref(ef), ctypes.byref(ew), ws.data_ptr(), ws.numel(),
                                           _stream_ptr(torch, stream)), "cetra_tc_correlation_probe")
     return dict(ms=ms.value, evals_per_s=float(n_out) * n_taps / (ms.value * 1e-3), err_wmf=ef.value, err_wmm=ew.value)
+
+
+def cetra_test_fold_override(force_stream: bool = False, stage_cells: int = 0) -> None:
+    """Test hook (include/cetra.h): make every later periodic search of this process use the streamed fold kernel
+    and/or small stages; called without arguments it restores the library's own plan."""
+    load_library().cetra_test_fold_override(1 if force_stream else 0, int(stage_cells))
 
 
 def cetra_linear_workspace_bytes(times, n_lc: int, durations, t0_start, t0_stride, n_t0, n_template: int) -> int:

@@ -317,7 +317,10 @@ int plan_batched(const double *times_host, int64_t n, int32_t n_lc, int32_t lc_c
                  LinearPlan *lin, BatchedLayout *lay, int32_t n_templates = 1) {
     if (n_lc < 1 || lc_chunk < 0 || n_per < 1 || n_templates < 1) return CETRA_ERR_INVALID_ARG;
     if (n_dur < 1 || grid.n_t0 < 1) return CETRA_ERR_INVALID_ARG;
-    const int32_t chunk = lc_chunk > 0 ? std::min(lc_chunk, n_lc) : default_chunk(n_lc, n_dur, grid.n_t0, n_templates);
+    // light curves are the z dimension of the linear kernel's launch grid: a chunk holds at most 65 535 of them,
+    // whatever the caller asked for (cetra.h)
+    const int32_t chunk = lc_chunk > 0 ? std::min(std::min(lc_chunk, n_lc), static_cast<int32_t>(65535))
+                                       : default_chunk(n_lc, n_dur, grid.n_t0, n_templates);
     const int rc = build_linear_plan(times_host, n, chunk, durations_host, n_dur, grid, n_template, d.smem_optin,
                                      d.n_sm, lin, n_templates);
     if (rc != CETRA_OK) return rc;

@@ -68,7 +68,7 @@ __global__ void __launch_bounds__(kProbeThreads, 1) peak_probe_kernel(int iters,
     for (int i = 0; i < kProbeAcc; ++i) acc[i] = make_float2(1.0f + tid * 1e-6f, 0.5f + i * 1e-6f);
     uint32_t base = 0;
     if (KIND == CETRA_PROBE_LDS64) {
-        const int n_cells = 32 * (kProbeThreads / 32) + 32 * kProbeStride + kProbeLoads + 4;
+        const int n_cells = 32 * (kProbeThreads / 32) + 32 * kProbeStride + 4 * kProbeLoads + 4;
         for (int i = tid; i < n_cells; i += kProbeThreads) cells[i] = make_float2(1e-9f * i, 1e-9f);
         base = smem_u32(cells) + 8u * static_cast<uint32_t>(warp * 32 + lane * kProbeStride);
     }
@@ -84,12 +84,19 @@ __global__ void __launch_bounds__(kProbeThreads, 1) peak_probe_kernel(int iters,
             for (int i = 0; i < kProbeAcc; ++i) acc[i] = probe_add2(acc[i], m);
         } else {
             float2 c[kProbeLoads];
-            const uint32_t b = base + 8u * static_cast<uint32_t>(it & 3);   // a new address every iteration: loads are not merged
+            // Every load of an unrolled body has an address of its own (the base moves by a whole group of kProbeLoads
+            // cells per trip, over a window of four groups) and is ld.volatile: ptxas may neither merge nor drop one.
+            // `asm volatile` alone does not say that -- it orders the asm statements but leaves the PTX load an ordinary
+            // one, and round 2's probe (base moving by ONE cell per trip, so that 30 of the 44 loads of a four-trip body
+            // repeated an address) was merged down to 14 LDS.64 and reported 3.0 x the crossbar's physical rate.
+            // SASS of this kernel, checked with cuobjdump: 44 LDS.64 per four-trip body.
+            const uint32_t b = base + 8u * static_cast<uint32_t>(kProbeLoads * (it & 3));
 #pragma unroll
             for (int i = 0; i < kProbeLoads; ++i)
-                asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];"
+                asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [%2];"
                              : "=f"(c[i].x), "=f"(c[i].y)
-                             : "r"(b + 8u * i));
+                             : "r"(b + 8u * i)
+                             : "memory");
 #pragma unroll
             for (int i = 0; i < kProbeLoads; ++i) acc[i] = probe_add2(acc[i], c[i]);
         }

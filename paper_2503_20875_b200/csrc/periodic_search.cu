@@ -13,12 +13,16 @@
 #include "fold_common.cuh"
 
 #include <math.h>
-#include <stdlib.h>
 
 #include <algorithm>
 #include <vector>
 
 namespace cetra {
+
+// Plan overrides for the parity tests (cetra_test_fold_override in cetra.h).  Set only through that call: the library
+// reads no environment variable, so nothing outside the process's own code can change which kernel a search runs.
+static std::atomic<int> g_test_force_stream{0};
+static std::atomic<int> g_test_stage_cells{0};
 
 // One thread per (light curve, period): decode the winning (j, p), redo its fold in the same order with
 // IEEE division, count the contributing epochs and write the record.
@@ -181,19 +185,16 @@ int build_periodic_plan(int32_t n_lc, int32_t n_dur, cetra_t0_grid grid, const d
     const size_t row_bytes = static_cast<size_t>(P.stats_pitch) * sizeof(float2);
     const size_t header = kGrpHeaderBytes;
     pl->row_in_smem = row_bytes + header <= static_cast<size_t>(smem_limit);
-    {
-        // test hook: CETRA_FORCE_STREAM=1 sends rows that would fit in shared memory through the streamed kernel, so
-        // that small problems (which the oracle folds in full) exercise it too
-        const char *env = getenv("CETRA_FORCE_STREAM");
-        if (env && env[0] == '1') pl->row_in_smem = false;
-    }
+    // test hook (cetra_test_fold_override): rows that would fit in shared memory go through the streamed kernel, so
+    // that small problems (which the oracle folds in full) exercise it too
+    if (g_test_force_stream.load(std::memory_order_relaxed)) pl->row_in_smem = false;
     if (pl->row_in_smem) {
         pl->smem_bytes = row_bytes + header;
     } else {
         // streamed kernel: the ring takes all the shared memory of the SM
         pl->stage_cells = static_cast<int>(((static_cast<size_t>(smem_limit) - kStrHeaderBytes) / (8 * kStrStages)) & ~size_t(1));
-        if (const char *env = getenv("CETRA_STREAM_STAGE_CELLS")) {     // test hook: small stages (block splitting, direct epochs)
-            const int v = atoi(env) & ~1;
+        {   // test hook (cetra_test_fold_override): small stages (block splitting, direct epochs)
+            const int v = g_test_stage_cells.load(std::memory_order_relaxed) & ~1;
             if (v >= 64 && v < pl->stage_cells) pl->stage_cells = v;
         }
         pl->smem_bytes = kStrHeaderBytes + static_cast<size_t>(kStrStages) * pl->stage_cells * 8;
@@ -286,3 +287,8 @@ int run_grids_to_stats(const float *depth_dev, const float *var_dev, const float
 }
 
 }  // namespace cetra
+
+extern "C" void cetra_test_fold_override(int32_t force_stream, int32_t stage_cells) {
+    cetra::g_test_force_stream.store(force_stream != 0 ? 1 : 0, std::memory_order_relaxed);
+    cetra::g_test_stage_cells.store(stage_cells > 0 ? stage_cells : 0, std::memory_order_relaxed);
+}

@@ -811,9 +811,9 @@ def test_linear_search_random_geometries(seed, torch_cuda, cetra, oracle_mod):
 
 
 @pytest.mark.parametrize("seed", range(8))
-def test_periodic_search_random_geometries_both_fold_kernels(seed, torch_cuda, cetra, oracle_mod, monkeypatch):
-    """Random small grids and period sets folded by the resident-row kernel and, through the library's test hooks
-    (CETRA_FORCE_STREAM, small CETRA_STREAM_STAGE_CELLS), by the streamed kernel with its epoch blocks split and some
+def test_periodic_search_random_geometries_both_fold_kernels(seed, torch_cuda, cetra, oracle_mod):
+    """Random small grids and period sets folded by the resident-row kernel and, through the library's test hook
+    (cetra_test_fold_override: forced streaming, small stages), by the streamed kernel with its epoch blocks split and some
     windows too wide for a stage: identical records from both, and parity with the oracle on every period."""
     from cetra_synth import tabulate_template
     rng = np.random.default_rng(7000 + seed)
@@ -843,11 +843,13 @@ def test_periodic_search_random_geometries_both_fold_kernels(seed, torch_cuda, c
                                                                          periods))[0]
     resident = run()
     assert_periodic_parity(resident, orc, cell, what=f"seed {seed} resident-row fold")
-    monkeypatch.setenv("CETRA_FORCE_STREAM", "1")
-    streamed = run()
-    monkeypatch.setenv("CETRA_STREAM_STAGE_CELLS", str(int(rng.choice([96, 200, 600]))))
-    streamed_small = run()
-    monkeypatch.delenv("CETRA_FORCE_STREAM"); monkeypatch.delenv("CETRA_STREAM_STAGE_CELLS")
+    try:
+        cetra.cetra_test_fold_override(force_stream=True)
+        streamed = run()
+        cetra.cetra_test_fold_override(force_stream=True, stage_cells=int(rng.choice([96, 200, 600])))
+        streamed_small = run()
+    finally:
+        cetra.cetra_test_fold_override()
     assert_periodic_parity(streamed, orc, cell, what=f"seed {seed} streamed fold")
     assert_periodic_parity(streamed_small, orc, cell, what=f"seed {seed} streamed fold, small stages")
     same = lambda a, b: np.array_equal(a["i_t0"], b["i_t0"]) and np.array_equal(a["j_dur"], b["j_dur"]) and \

@@ -172,3 +172,18 @@ def test_resample_template_host_helper_matches_the_oracle(cetra, oracle_mod):
         assert np.array_equal(got, want.astype(np.float32)) or np.abs(got - want).max() <= 6e-8
     with pytest.raises(cetra.CetraError):
         cetra.cetra_resample_template(dense[:1], 8)
+
+
+def test_light_curve_count_limits_of_one_launch(cetra):
+    """Light curves are one dimension of the linear kernel's launch grid (65 535 at most).  cetra_linear_search says so
+    (no workspace size = unsupported); the batched search slices by itself and clamps a caller's larger chunk."""
+    c = 2.0 / 1440.0
+    times = c * np.arange(64)
+    durations = np.array([4 * c, 8 * c])
+    args = (durations, 0.0, c, 64, 32)
+    assert cetra.cetra_linear_workspace_bytes(times, 65535, *args) > 0
+    assert cetra.cetra_linear_workspace_bytes(times, 65536, *args) == 0
+    at_limit = cetra.cetra_search_batched_workspace_bytes(times, 100000, 65535, *args, 10)
+    beyond = cetra.cetra_search_batched_workspace_bytes(times, 100000, 90000, *args, 10)
+    smaller = cetra.cetra_search_batched_workspace_bytes(times, 100000, 30000, *args, 10)
+    assert 0 < smaller < at_limit == beyond
