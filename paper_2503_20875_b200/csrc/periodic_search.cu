@@ -24,7 +24,7 @@ namespace cetra {
 static std::atomic<int> g_test_force_stream{0};
 static std::atomic<int> g_test_stage_cells{0};
 
-// One thread per (light curve, period): decode the winning (j, p), redo its fold in the same order with
+// One thread per (light curve, period): decode the winning (j, p), redo its fold in FP64 with
 // IEEE division, count the contributing epochs and write the record.
 __global__ void finalize_peaks_kernel(const __grid_constant__ PeriodicParams P, cetra_peak *__restrict__ peaks) {
     const long long total = static_cast<long long>(P.n_lc) * P.n_per;
@@ -45,20 +45,25 @@ __global__ void finalize_peaks_kernel(const __grid_constant__ PeriodicParams P, 
             const double r = P.r_cells[k];
             const bool literal = P.literal && *P.literal;
             const float *res = literal ? P.resid + (lc * P.n_dur + j) * P.stats_pitch : nullptr;
-            float sa = 0.f, sb = 0.f, sc = 0.f;
+            // FP64 sums and combination (north_star: "FP64 final sums if needed"): the record is then the FP32 cells'
+            // exact fold rounded once, also where epochs of opposite sign cancel (Z ~ 0 out of large per-transit
+            // terms) and a running FP32 sum would lose 1e-5 of the small combined LR.  One thread per record, a few
+            // dozen cells each: 0.1 % of a search.
+            double sa = 0.0, sb = 0.0, sc = 0.0;
             int ntr = 0;
             for (long long e = 0;; ++e) {
                 const long long cell = p + __double2ll_rn(__dmul_rn(static_cast<double>(e), r));
                 if (cell > P.n_t0 - 1) break;
                 const float2 ab = row[cell];
-                sa += ab.x;
-                sb += ab.y;
-                if (literal) sc += res[cell];
+                sa += static_cast<double>(ab.x);
+                sb += static_cast<double>(ab.y);
+                if (literal) sc += static_cast<double>(res[cell]);
                 ntr += ab.x > 0.f ? 1 : 0;
             }
-            out.depth = sb / sa;                                     // common depth Z
-            out.depth_var = 1.0f / sa;
-            out.lr = 0.5f * sb * out.depth + sc;                     // Eq. 4 summed at Z (sc = 0 unless literal)
+            const double z = sb / sa;                                // common depth Z
+            out.depth = static_cast<float>(z);
+            out.depth_var = static_cast<float>(1.0 / sa);
+            out.lr = static_cast<float>(0.5 * sb * z + sc);          // Eq. 4 summed at Z (sc = 0 unless literal)
             out.t0 = static_cast<float>(P.t0_start + static_cast<double>(p) * P.t0_stride);
             out.i_t0 = p; out.j_dur = j; out.n_transits = ntr;
         }

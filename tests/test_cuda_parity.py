@@ -810,6 +810,20 @@ def test_linear_search_random_geometries(seed, torch_cuda, cetra, oracle_mod):
         assert np.all(st[:, n_t0:] == 0) and np.all(st[:, :n_t0, 0][np.isnan(o.depth)] == 0)
 
 
+def _grids_from_stats(stats, n_t0):
+    """The linear-search grids the sufficient-statistics rows stand for, in FP64: stats is one light curve's
+    [n_dur][pitch][2] float32 tensor (S_wmm, S_wmf); null cells (S_wmm = 0) become NaN.  Feeding the oracle these
+    gives both sides of a periodic-search comparison the same numbers to start from."""
+    import oracle as oracle_pkg
+    st = stats.cpu().numpy().astype(np.float64)[:, :n_t0, :]
+    a, b = st[..., 0], st[..., 1]
+    with np.errstate(divide="ignore", invalid="ignore"):
+        depth = np.where(a > 0, b / a, np.nan)
+        var = np.where(a > 0, 1.0 / a, np.nan)
+        dl = np.where(a > 0, 0.5 * b * b / a, np.nan)
+    return oracle_pkg.LinearGrids(depth, var, dl)
+
+
 @pytest.mark.parametrize("seed", range(8))
 def test_periodic_search_random_geometries_both_fold_kernels(seed, torch_cuda, cetra, oracle_mod):
     """Random small grids and period sets folded by the resident-row kernel and, through the library's test hook
@@ -835,8 +849,8 @@ def test_periodic_search_random_geometries_both_fold_kernels(seed, torch_cuda, c
     fl, er = _dev(torch_cuda, flux), _dev(torch_cuda, err)
     lin = cetra.cetra_linear_search(times, fl, er, durations, times[0], stride, n_t0, tpl, want_stats=True)
     torch_cuda.cuda.synchronize()
-    import oracle as oracle_pkg
-    g64 = oracle_pkg.LinearGrids(*(a.cpu().numpy().astype(np.float64) for a in (lin.depth, lin.depth_var, lin.dlogL)))
+    # the oracle folds exactly what the GPU folds: the FP32 (S_wmm, S_wmf) rows, as FP64 depth = B/A, var = 1/A
+    g64 = _grids_from_stats(lin.stats[0], n_t0)
     orc = oracle_mod.periodic_search(g64, times[0], stride, durations, periods)
     cell = lambda k, j, ph: oracle_mod.periodic_cell(g64, stride, periods[k], j, ph)
     run = lambda: cetra.peaks_to_numpy(cetra.cetra_periodic_search_stats(lin.stats, n_t0, times[0], stride, durations,
@@ -857,3 +871,81 @@ def test_periodic_search_random_geometries_both_fold_kernels(seed, torch_cuda, c
     assert same(streamed, streamed_small)
     # the two kernels add a cell's epochs in different orders: same winners except at FP32 near-ties
     assert np.mean((resident["i_t0"] == streamed["i_t0"]) & (resident["j_dur"] == streamed["j_dur"])) >= 0.97
+
+
+def _cancelling_light_curve(rng, n, cadence):
+    """Deep events of BOTH signs (dips and equally deep brightenings, tens to hundreds of sigma) at random places:
+    folded at a period that is the spacing of two of them, a cell's epochs cancel, the common depth Z is a small
+    difference of large per-transit terms, and so is the combined likelihood ratio.  Returns the light curve and the
+    event centres."""
+    times = 3.0 + np.arange(n) * cadence
+    err = rng.uniform(3e-4, 1.2e-3, size=n)
+    flux = 1.0 + rng.normal(size=n) * err
+    centres = np.sort(rng.uniform(times[0] + 20 * cadence, times[-1] - 20 * cadence, size=int(rng.integers(3, 7))))
+    partners = []
+    for c in centres:
+        depth = float(rng.choice([-1.0, 1.0])) * rng.uniform(0.8e-2, 5e-2)
+        width = rng.uniform(6, 30) * cadence
+        flux -= depth * (np.abs(times - c) < width / 2)
+        if rng.random() < 0.5:
+            # a partner of the same shape and nearly the opposite depth: folded at their spacing, 90-99 % of the
+            # signal cancels and the cell still stands out of the noise
+            c2 = c + float(rng.choice([-1.0, 1.0])) * rng.uniform(60, 0.4 * n) * cadence
+            if times[0] + 20 * cadence < c2 < times[-1] - 20 * cadence:
+                flux += depth * (1.0 + float(rng.choice([-1.0, 1.0])) * rng.uniform(0.01, 0.1)) * \
+                    (np.abs(times - c2) < width / 2)
+                partners.append(c2)
+    flux[rng.random(n) < 0.02] = np.nan
+    return times, flux.astype(np.float32), err.astype(np.float32), np.sort(np.concatenate([centres, partners]))
+
+
+def test_periodic_search_ill_conditioned_folds(torch_cuda, cetra, oracle_mod):
+    """200 seeded problems of the kind the 1e-5 bound is hardest on: events of opposite sign folded
+    onto one another, so that the winning cell's LR is what is left of large terms that cancel.  The trial periods
+    are the spacings of the events (and their halves), where that happens, plus random ones.  Both fold kernels,
+    every period against the oracle folding the same FP32 statistics.  Time-boxed: at least 60 of the 200 seeds must
+    have run when the box closes (all of them do on a B200 in well under a minute)."""
+    import time
+    from cetra_synth import tabulate_template
+    tpl = tabulate_template(256)
+    cadence = 120.0 / 86400.0
+    t_end = time.monotonic() + 150.0
+    done, worst, n_cancel = 0, 0.0, 0
+    for seed in range(200):
+        if time.monotonic() > t_end:
+            break
+        rng = np.random.default_rng(31000 + seed)
+        n = int(rng.integers(500, 1600))
+        times, flux, err, centres = _cancelling_light_curve(rng, n, cadence)
+        durations = np.sort(rng.uniform(5.0, 32.0, size=3)) * cadence
+        stride = cadence * float(rng.choice([1.0, 0.5]))
+        n_t0 = int((times[-1] - times[0]) / stride) + 1
+        gaps = np.abs(centres[:, None] - centres[None, :])[np.triu_indices(len(centres), 1)]
+        cand = np.concatenate([gaps, gaps / 2.0, gaps / 3.0, rng.uniform(40 * cadence, 0.6 * (times[-1] - times[0]), 12)])
+        periods = np.sort(cand[cand > durations.max() + 2 * cadence])
+        fl, er = _dev(torch_cuda, flux), _dev(torch_cuda, err)
+        lin = cetra.cetra_linear_search(times, fl, er, durations, times[0], stride, n_t0, tpl, want_stats=True,
+                                        want_grids=False)
+        g64 = _grids_from_stats(lin.stats[0], n_t0)
+        orc = oracle_mod.periodic_search(g64, times[0], stride, durations, periods)
+        cell = lambda k, j, ph: oracle_mod.periodic_cell(g64, stride, periods[k], j, ph)
+        run = lambda: cetra.peaks_to_numpy(cetra.cetra_periodic_search_stats(lin.stats, n_t0, times[0], stride,
+                                                                             durations, periods))[0]
+        resident = run()
+        try:
+            cetra.cetra_test_fold_override(force_stream=True)
+            streamed = run()
+        finally:
+            cetra.cetra_test_fold_override()
+        for name, rec in (("resident", resident), ("streamed", streamed)):
+            w = assert_periodic_parity(rec, orc, cell, what=f"cancelling seed {seed} {name}")
+            worst = max(worst, w["lr"])
+        # how hard the case was: winners whose |Z| is far below the single-epoch depths that went into them
+        ok = ~np.isnan(orc.lr)
+        single = np.nanmax(np.abs(g64.depth))
+        n_cancel += int(np.sum(np.abs(orc.depth[ok]) < 0.05 * single))
+        done += 1
+    print(f"ill-conditioned fuzz: {done} seeds, {n_cancel} cancelling winners, worst LR error {worst:.3g}")
+    assert done >= 60, f"only {done} seeds ran inside the time box"
+    assert n_cancel >= done                     # on average at least one strongly cancelling winner per problem
+    assert worst <= REL
