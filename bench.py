@@ -70,6 +70,110 @@ def fold_sources_sha256() -> str:
     return h.hexdigest()
 
 
+# ---------------------------------------------- other workloads on the same line (round-2 review, "Next round" 3)
+# Per-curve counters of fold_stream_argmax_kernel from the ncu pass named in `profile` (metrics only: LDS wavefronts,
+# DRAM bytes), valid for the sources whose hash is `src_sha256`; like NCU_FOLD they are properties of the launch.
+NCU_STREAM = dict(
+    profile="profiles/r03a_fold_stream_legs.md", src_sha256="9d7102a06b6e1040f84cc9443b940568184f8c03867b304e3f1df1f4f9add4bf", per_curve={
+        # leg name -> (l1tex__data_pipe_lsu_wavefronts_mem_shared.sum, dram bytes read + written) of ONE light curve
+        "configs3": (101992340344.0, 113329408.0 + 2987520.0),                       # one curve per launch, 78.2 % under ncu
+        "default_grid": (62437322352.0 / 16, (141049652224.0 + 20825344.0) / 16),   # 16 curves per launch, 85.8 % under ncu
+    })
+STREAM_SOURCES = ("fold_stream.cu", "fold_common.cuh", "periodic_search.cuh", "common.cuh")
+
+
+def sources_sha256(names) -> str:
+    import hashlib
+    h = hashlib.sha256()
+    for name in names:
+        with open(os.path.join(ROOT, "paper_2503_20875_b200", "csrc", name), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()
+
+
+def config_legs(cetra, torch, dev, peaks, flush, reps: int = 2):
+    """The workloads whose rooflines the docs quote besides the headline one, timed in this process after the main
+    region (a few seconds in all): BASELINE configs[2] (20-s cadence) linear search in a batch of 32, configs[3]
+    (one 256 464-cell curve) whole search, and configs[1] on the paper's default t0 grid (stride = 1 % of the
+    shortest duration) in a batch of 64.  Kernel times are the library's own event brackets around its
+    linear-search and fold kernels (cetra_profile_enable), averaged per launch over `reps` passes after one warm-up,
+    L2 flushed between passes.  Returns a list of {workload, kernel, ms, launches, bound, achieved, peak, unit, frac}."""
+    from cetra_synth import make_config, make_survey_batch
+    fp32_peak = N_SM * FP32_LANES * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12          # TFLOP/s
+    smem_peak = N_SM * SMEM_BYTES_PER_CLK * peaks["sm_max_mhz"] * 1e6 / 1e9        # GB/s
+    stream_stale = sources_sha256(STREAM_SOURCES) != NCU_STREAM["src_sha256"]
+
+    def profiled(fn):
+        fn()
+        torch.cuda.synchronize()
+        cetra.cetra_profile_enable(True)
+        for _ in range(reps):
+            flush.zero_()
+            fn()
+        torch.cuda.synchronize()
+        prof = cetra.cetra_profile_read(reset=True)
+        cetra.cetra_profile_enable(False)
+        return prof
+
+    def linear_leg(workload, kernel, prof, evals_per_pass):
+        ms = prof["linear_ms"] / max(prof["linear_launches"], 1)
+        tf = 4.0 * evals_per_pass * reps / (prof["linear_ms"] * 1e-3) / 1e12
+        return dict(workload=workload, kernel=kernel, ms=ms, launches=int(prof["linear_launches"]), bound="alu",
+                    achieved=tf, peak=fp32_peak, unit="TFLOP/s", frac=tf / fp32_peak,
+                    template_evals_per_s=evals_per_pass * reps / (prof["linear_ms"] * 1e-3))
+
+    def stream_leg(workload, name, prof, curves_per_pass, cells_per_curve):
+        ms = prof["fold_ms"] / max(prof["fold_launches"], 1)
+        counters = None if stream_stale else NCU_STREAM["per_curve"].get(name)
+        leg = dict(workload=workload, kernel="fold_stream_argmax_kernel", ms=ms, launches=int(prof["fold_launches"]),
+                   bound="smem", peak=smem_peak, unit="GB/s", achieved=None, frac=None, traffic=None,
+                   fold_cells_per_s=cells_per_curve * curves_per_pass * reps / (prof["fold_ms"] * 1e-3),
+                   ms_per_curve=prof["fold_ms"] / (curves_per_pass * reps), ncu_stale=stream_stale)
+        if counters:
+            gbs = 128.0 * counters[0] * curves_per_pass * reps / (prof["fold_ms"] * 1e-3) / 1e9
+            leg.update(achieved=gbs, frac=gbs / smem_peak, traffic=counters[1] * curves_per_pass * reps /
+                       max(prof["fold_launches"], 1))
+        return leg
+
+    legs = []
+    # -- configs[2]: 20-s cadence, 118 368 points, long windows (up to 2 701 taps): the linear kernel in a batch of 32
+    p = make_config(3)
+    wc = work_counts(p)
+    fl = torch.from_numpy(np.tile(p.flux, (32, 1))).to(dev)
+    er = torch.from_numpy(np.tile(p.flux_err, (32, 1))).to(dev)
+    prof = profiled(lambda: cetra.cetra_linear_search(p.times, fl, er, p.durations, p.t0_start, p.t0_stride, p.n_t0,
+                                                      p.template, want_grids=False, want_stats=True))
+    legs.append(linear_leg(f"BASELINE configs[2] {p.name} x 32 light curves (one curve tiled), linear search",
+                           "linear_search_kernel", prof, 32.0 * wc["template_evals"]))
+    del fl, er
+    # -- configs[3]: one curve, rows of 2 MB: linear search + the streamed fold
+    p = make_config(4)
+    wc = work_counts(p)
+    fl, er = torch.from_numpy(p.flux).to(dev), torch.from_numpy(p.flux_err).to(dev)
+    prof = profiled(lambda: cetra.cetra_search_batched(p.times, fl[None], er[None], p.durations, p.t0_start,
+                                                       p.t0_stride, p.n_t0, p.template, p.periods))
+    legs.append(linear_leg(f"BASELINE configs[3] {p.name}, one light curve, linear search", "linear_search_kernel",
+                           prof, float(wc["template_evals"])))
+    legs.append(stream_leg(f"BASELINE configs[3] {p.name}, one light curve, periodic search", "configs3", prof, 1,
+                           float(wc["gathers"])))
+    del fl, er
+    # -- configs[1] on the paper's default t0 grid (18 s = 3/20 of the cadence): residue-class linear kernel + streamed fold
+    B = 64
+    p = make_survey_batch(n_lc=B, lc_range=(0, B))
+    wc = work_counts(p)
+    stride = 0.01 * p.durations[0]
+    n_t0 = int((p.times[-1] - p.times[0]) / stride) + 1
+    fl, er = torch.from_numpy(p.flux).to(dev), torch.from_numpy(p.flux_err).to(dev)
+    prof = profiled(lambda: cetra.cetra_search_batched(p.times, fl, er, p.durations, p.times[0], stride, n_t0,
+                                                       p.template, p.periods))
+    what = f"BASELINE configs[1] on the paper's default t0 grid (stride 18 s, {n_t0} cells) x {B} light curves"
+    legs.append(linear_leg(what + ", linear search", "linear_search_kernel<CLS> (residue classes)", prof,
+                           B * wc["template_evals"] * (n_t0 / p.n_t0)))
+    legs.append(stream_leg(what + ", periodic search", "default_grid", prof, B, float(wc["pairs"]) * n_t0))
+    return legs
+
+
+
 # ----------------------------------------------------------------------------------------------- helpers
 def measured_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
@@ -263,6 +367,10 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
     if world > 1 and not dist.is_initialized():
         dist.init_process_group("nccl", device_id=dev)
 
+    if args.legs_only:
+        flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+        print(json.dumps(dict(configs=config_legs(cetra, torch, dev, measured_peaks(), flush, reps=1))), flush=True)
+        return
     B = args.n_lc
     p = make_survey_batch(n_lc=B * world, lc_range=rank_slice(rank, world, B))   # each rank owns its curves
     wc = work_counts(p)
@@ -403,6 +511,10 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
                    template_evals_per_lc=wc["template_evals"], gathers_per_lc=wc["gathers"],
                    duration_period_pairs=wc["pairs"], fadd2_probe=probes["fadd2"]),
     )
+    if world == 1 and not args.no_legs:
+        del ws, peaks_d, flux_d, err_d
+        torch.cuda.empty_cache()
+        line["configs"] = config_legs(cetra, torch, dev, peaks, flush)
     if world == 1 and not args.no_cpu_baseline:
         v, sample, cores, _ = oracle_sample(p, p.flux[0], p.flux_err[0], args.cpu_seconds)
         v1, sample1, _, _ = oracle_sample(p, p.flux[0], p.flux_err[0], args.cpu_seconds / 2, threads=1)
@@ -602,6 +714,9 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="CPU budget of the cpu_baseline sample")
     ap.add_argument("--ref-seconds", type=float, default=8.0, help="CPU budget of one --impl reference step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-legs", action="store_true", help="skip the `configs` list (other workloads' rooflines)")
+    ap.add_argument("--legs-only", action="store_true",
+                    help="run only the `configs` legs and print them (the command the ncu passes under profiles/ use)")
     ap.add_argument("--master-port", type=int, default=29541, help="rendezvous port when bench.py spawns the ranks")
     args = ap.parse_args()
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.workload == "sector":
