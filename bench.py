@@ -647,14 +647,17 @@ def run_configs(args):
                                   periodic_ms=ogp_ms, fold_algorithmic_gbs=og_bytes / (ogp_ms * 1e-3) / 1e9,
                                   light_curves_per_s=1e3 / (og_ms + ogp_ms))), flush=True)
     # setup kernels: resampling 64 irregular light curves of 200 000 observations (HBM-bound streaming)
-    t, f, e = make_irregular_batch(n_lc=64, n=200000)
-    td, fd, ed = (torch.from_numpy(a).to(dev) for a in (t, f, e))
-    t_start, c, n_out = cetra.cetra_resample_grid(t, 0.0, 0.25)
-    rs_ms = med_ms(lambda: cetra.cetra_resample(td, fd, ed, t_start, c, n_out), max(3, args.steps))
-    moved = f.nbytes + e.nbytes + t.nbytes + 64 * n_out * (16 * 2 + 8)       # in + FP64 sums written/read + out
-    print(json.dumps(dict(workload="cetra_resample, 64 curves x %d observations -> %d points" % (t.shape[0], n_out),
-                          ms=rs_ms, algorithmic_gbs=moved / (rs_ms * 1e-3) / 1e9,
-                          frac_hbm=moved / (rs_ms * 1e-3) / 1e9 / peaks_hw["hbm_gbs"])), flush=True)
+    for shuffle in (False, True):
+        t, f, e = make_irregular_batch(n_lc=64, n=200000, shuffle=shuffle)
+        td, fd, ed = (torch.from_numpy(a).to(dev) for a in (t, f, e))
+        t_start, c, n_out = cetra.cetra_resample_grid(t, 0.0, 0.25)
+        rs_ms = med_ms(lambda: cetra.cetra_resample(td, fd, ed, t_start, c, n_out), max(3, args.steps))
+        moved = f.nbytes + e.nbytes + t.nbytes + 64 * n_out * 8     # every input read once, every output written once
+        print(json.dumps(dict(workload="cetra_resample, 64 curves x %d observations -> %d points, input %s"
+                                       % (t.shape[0], n_out, "in random order (4-byte gathers: 8 x the bytes through "
+                                          "L2)" if shuffle else "in time order"),
+                              ms=rs_ms, algorithmic_gbs=moved / (rs_ms * 1e-3) / 1e9,
+                              frac_hbm=moved / (rs_ms * 1e-3) / 1e9 / peaks_hw["hbm_gbs"])), flush=True)
 
 
 # --------------------------------------------------------- tensor-core variant of the windowed sums (diagnostic)

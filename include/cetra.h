@@ -255,15 +255,20 @@ int cetra_resample_template(const float *model_host, int32_t n_model, float *tem
  *     times_dev              [n_in] float64 DEVICE (the irregular timestamps are a large array)
  *     flux_dev, flux_err_dev [n_lc][n_in] dtype, sharing times_dev
  *     flux_out_dev, flux_err_out_dev [n_lc][n_out] dtype (same dtype as the input); n_in = 0 gives an all-null grid
- *     workspace              cetra_resample_workspace_bytes(n_lc, n_out): FP64 sums per output point
- * The sums are FP64 atomics: the result does not depend on the order of the input beyond FP64 rounding.
+ *     workspace              cetra_resample_workspace_bytes(n_in, n_lc, n_out): four int32 arrays (the output point of
+ *                            every observation, the observations of every point, counts, offsets); it does not grow
+ *                            with n_lc, because the light curves share the timestamps
+ * The observation -> point lists are built once per call for all light curves, and each (light curve, point) sum adds
+ * its observations in ascending input index in FP64: no floating-point atomics, so the result is bit-identical from
+ * run to run and equals a sequential pass over the input; it does not depend on the order of the input beyond FP64
+ * rounding.  Limits: n_in < 2^31, n_out < 2^31 - 1 (CETRA_ERR_UNSUPPORTED beyond).
  * ------------------------------------------------------------------------------------------ */
 int cetra_median_cadence(const double *times_host, int64_t n, double *cadence);
 
 int cetra_resample_grid(const double *times_host, int64_t n, double cadence, double pad_days,
                         double *t_start, double *cadence_out, int64_t *n_out);
 
-size_t cetra_resample_workspace_bytes(int32_t n_lc, int64_t n_out);
+size_t cetra_resample_workspace_bytes(int64_t n_in, int32_t n_lc, int64_t n_out);
 
 int cetra_resample(const double *times_dev, const void *flux_dev, const void *flux_err_dev, cetra_dtype dtype,
                    int64_t n_in, int32_t n_lc, double t_start, double cadence, int64_t n_out,
@@ -273,8 +278,8 @@ int cetra_resample(const double *times_dev, const void *flux_dev, const void *fl
 /* ------------------------------------------------------------------------------------------
  * cetra_resample for callers that have no device memory to give as a workspace.
  *
- * Who this is for.  cetra_resample needs cetra_resample_workspace_bytes() of device scratch (one pair of FP64 sums
- * per output point).  Some callers cannot produce that: code that runs inside somebody else's memory budget and is
+ * Who this is for.  cetra_resample needs cetra_resample_workspace_bytes() of device scratch (index lists that grow
+ * with the number of observations).  Some callers cannot produce that: code that runs inside somebody else's memory budget and is
  * handed its input and output buffers but no allocator (a plug-in stage of a pipeline, a worker whose device pool
  * was carved up front and is full), code on a path where cudaMalloc is not allowed because it synchronises the
  * whole device (a latency-critical service loop, a region other threads are capturing or timing), and code in a
@@ -290,8 +295,9 @@ int cetra_resample(const double *times_dev, const void *flux_dev, const void *fl
  * CETRA_ERR_STATIC_LIMIT before anything is enqueued; split the light curves over several calls, or use
  * cetra_resample with a workspace.  cetra_resample_static_max_points() returns the limit at run time.
  *
- * Arguments, arithmetic and results are cetra_resample's (same kernels, same FP64 atomic sums): the two agree to
- * FP64 rounding of the sums, i.e. after rounding to the output dtype to within one unit in the last place.
+ * Arguments and results are cetra_resample's.  The sums here are FP64 atomic adds into the fixed array (one pair per
+ * output point, which is what bounds n_lc * n_out), so their order varies from run to run: the two entry points agree
+ * to FP64 rounding of the sums, i.e. after rounding to the output dtype to within one unit in the last place.
  * The call makes no cudaMalloc / cudaFree and calls nothing that allocates; it enqueues one memset of the part of
  * the array it uses and two kernels on `cuda_stream` and returns without synchronising.
  *

@@ -130,7 +130,7 @@ def load_library() -> ctypes.CDLL:
     lib.cetra_resample_grid.restype = ctypes.c_int
     lib.cetra_resample_grid.argtypes = [dp, i64, ctypes.c_double, ctypes.c_double, dp, dp, ctypes.POINTER(i64)]
     lib.cetra_resample_workspace_bytes.restype = sz
-    lib.cetra_resample_workspace_bytes.argtypes = [i32, i64]
+    lib.cetra_resample_workspace_bytes.argtypes = [i64, i32, i64]
     lib.cetra_resample.restype = ctypes.c_int
     lib.cetra_resample.argtypes = [vp, vp, vp, ctypes.c_int, i64, i32, ctypes.c_double, ctypes.c_double, i64,
                                    vp, vp, vp, sz, vp]
@@ -626,7 +626,7 @@ def cetra_resample(times_dev, flux, flux_err, t_start: float, cadence: float, n_
     if not (times_dev.is_cuda and times_dev.dtype == torch.float64 and times_dev.numel() == n_in):
         raise TypeError("times_dev must be a float64 CUDA tensor with one entry per observation")
     times_dev = times_dev.contiguous()
-    nbytes = int(lib.cetra_resample_workspace_bytes(n_lc, int(n_out)))
+    nbytes = int(lib.cetra_resample_workspace_bytes(n_in, n_lc, int(n_out)))
     ws = _workspace(torch, nbytes, flux.device, workspace)
     out_f = torch.empty((n_lc, int(n_out)), dtype=flux.dtype, device=flux.device)
     out_e = torch.empty_like(out_f)

@@ -15,6 +15,8 @@
 namespace cetra {
 
 // ------------------------------------------------------------------------------------------ resample
+// Atomic-sum form, now used by cetra_resample_static only (its scratch is the fixed FP64 sums array; the fixed-order
+// path below needs scratch that grows with the number of observations).
 // One thread per (light curve, observation): atomically add (w, w f) to the observation's output point.
 template <typename T>
 __global__ void resample_accumulate_kernel(const double *__restrict__ times, const T *__restrict__ flux,
@@ -53,6 +55,231 @@ __global__ void resample_finalize_kernel(const double2 *__restrict__ sums, long 
         } else {
             flux_out[idx] = static_cast<T>(__longlong_as_double(0x7ff8000000000000LL));   // null flux
             err_out[idx] = static_cast<T>(__longlong_as_double(0x7ff0000000000000LL));    // infinite error
+        }
+    }
+}
+
+// ------------------------------------------------------------------- resample, fixed summation order
+// cetra_resample's own path (round 3).  All light curves of a call share the timestamps, so which
+// output point an observation falls on is the same for every curve: it is worked out ONCE, as a compressed list of
+// observation indices per output point (count -> exclusive scan -> fill -> sort each point's few indices), and then the
+// sum kernel adds each (light curve, output point)'s observations in ascending input index in FP64.  No floating-point
+// atomics: the result is bit-identical from run to run and equal to a sequential loop over the input (the oracle's
+// order); each flux / error value is read once and each output written once.
+
+// Observation -> output point (R21, FP64), -1 for a non-finite or off-grid time; counts per point (integer atomics).
+__global__ void resample_cells_kernel(const double *__restrict__ times, int n_in, double t_start, double cadence,
+                                      int n_out, int *__restrict__ cell_of, int *__restrict__ count) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_in; i += gridDim.x * blockDim.x) {
+        const double t = times[i];
+        int c = -1;
+        if (isfinite(t)) {
+            const double cell = floor(__dadd_rn(__ddiv_rn(__dsub_rn(t, t_start), cadence), 0.5));
+            if (cell >= 0.0 && cell < static_cast<double>(n_out)) c = static_cast<int>(cell);
+        }
+        cell_of[i] = c;
+        if (c >= 0) atomicAdd(count + c, 1);
+    }
+}
+
+// Exclusive scan of the counts in two launches over tiles of kScanTile points (a single CTA walking 2e5 counts was
+// latency-bound at 0.3 ms, ncu r03b): first each tile's total, then every tile finds its base by adding the totals
+// of the tiles before it (a few dozen numbers for a sector) and scans itself.  offsets[n_out + 1]; the counts are
+// replaced by the offsets so that the fill can use them as cursors.
+constexpr int kScanThreads = 256;
+constexpr int kScanTile = 4 * kScanThreads;
+
+__device__ __forceinline__ int block_sum_256(int v, int *s_warp) {          // total over the CTA, to every thread
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    __syncthreads();                                                        // s_warp may still be read from a previous use
+    if (lane == 0) s_warp[warp] = v;
+    __syncthreads();
+    int t = 0;
+#pragma unroll
+    for (int w = 0; w < kScanThreads / 32; ++w) t += s_warp[w];
+    return t;
+}
+
+__global__ void __launch_bounds__(kScanThreads) resample_tile_sums_kernel(const int *__restrict__ count, int n_out,
+                                                                         int *__restrict__ tile_sum) {
+    __shared__ int s_warp[kScanThreads / 32];
+    const int base = blockIdx.x * kScanTile + threadIdx.x * 4;
+    int v = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) v += base + k < n_out ? count[base + k] : 0;
+    const int t = block_sum_256(v, s_warp);
+    if (threadIdx.x == 0) tile_sum[blockIdx.x] = t;
+}
+
+__global__ void __launch_bounds__(kScanThreads) resample_scan_kernel(int *__restrict__ count,
+                                                                    const int *__restrict__ tile_sum,
+                                                                    int *__restrict__ offsets, int n_out) {
+    __shared__ int s_warp[kScanThreads / 32];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    int before = 0;
+    for (int b = tid; b < static_cast<int>(blockIdx.x); b += kScanThreads) before += tile_sum[b];
+    const int tile_base = block_sum_256(before, s_warp);
+    const int base = blockIdx.x * kScanTile + tid * 4;
+    int c[4], sum = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        c[k] = base + k < n_out ? count[base + k] : 0;
+        sum += c[k];
+    }
+    int incl = sum;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int o = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += o;
+    }
+    __syncthreads();
+    if (lane == 31) s_warp[warp] = incl;
+    __syncthreads();
+    int run = tile_base + incl - sum;
+    for (int w = 0; w < warp; ++w) run += s_warp[w];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        if (base + k < n_out) {
+            offsets[base + k] = run;
+            count[base + k] = run;
+        }
+        run += c[k];
+        if (base + k == n_out - 1) offsets[n_out] = run;
+    }
+}
+
+__global__ void resample_fill_kernel(const int *__restrict__ cell_of, int n_in, int *__restrict__ cursor,
+                                     int *__restrict__ order) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_in; i += gridDim.x * blockDim.x) {
+        const int c = cell_of[i];
+        if (c >= 0) order[atomicAdd(cursor + c, 1)] = i;
+    }
+}
+
+// The fill leaves each point's indices in arrival order; put them in ascending order (the fixed summation order).
+// One thread per output point: a point holds a handful of observations (insertion sort), heapsort beyond 16 so that
+// a degenerate grid (everything in one point) costs m log m, not m^2.
+__global__ void resample_sort_kernel(const int *__restrict__ offsets, int n_out, int *__restrict__ order) {
+    for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < n_out; c += gridDim.x * blockDim.x) {
+        const int lo = offsets[c], m = offsets[c + 1] - lo;
+        if (m < 2) continue;
+        int *a = order + lo;
+        if (m <= 16) {
+            for (int i = 1; i < m; ++i) {
+                const int v = a[i];
+                int k = i - 1;
+                while (k >= 0 && a[k] > v) { a[k + 1] = a[k]; --k; }
+                a[k + 1] = v;
+            }
+            continue;
+        }
+        auto sift = [a](int root, int end) {                     // max-heap on a[0 .. end)
+            const int v = a[root];
+            for (;;) {
+                int child = 2 * root + 1;
+                if (child >= end) break;
+                if (child + 1 < end && a[child + 1] > a[child]) ++child;
+                if (a[child] <= v) break;
+                a[root] = a[child];
+                root = child;
+            }
+            a[root] = v;
+        };
+        for (int i = m / 2 - 1; i >= 0; --i) sift(i, m);
+        for (int end = m - 1; end > 0; --end) {
+            const int t = a[0]; a[0] = a[end]; a[end] = t;
+            sift(0, end);
+        }
+    }
+}
+
+// Inverse-variance weighted mean of an output point's valid observations, added in ascending input index; formal
+// error; null (NaN, +inf) where there is none.
+template <typename T>
+__device__ __forceinline__ void resample_point(const T *__restrict__ fl, const T *__restrict__ er,
+                                               const int *__restrict__ order, int lo, int m, T *flux_out, T *err_out) {
+    double sw = 0.0, swf = 0.0;
+    for (int k = lo; k < lo + m; ++k) {
+        const int i = order[k];
+        const double f = static_cast<double>(fl[i]), e = static_cast<double>(er[i]);
+        if (!(isfinite(f) && isfinite(e) && e > 0.0)) continue;                   // null observation (R8)
+        const double w = __ddiv_rn(1.0, __dmul_rn(e, e));
+        sw = __dadd_rn(sw, w);
+        swf = __dadd_rn(swf, __dmul_rn(w, f));
+    }
+    if (sw > 0.0) {
+        *flux_out = static_cast<T>(__ddiv_rn(swf, sw));
+        *err_out = static_cast<T>(__dsqrt_rn(__ddiv_rn(1.0, sw)));
+    } else {
+        *flux_out = static_cast<T>(__longlong_as_double(0x7ff8000000000000LL));
+        *err_out = static_cast<T>(__longlong_as_double(0x7ff0000000000000LL));
+    }
+}
+
+// One CTA per 256 output points and group of G light curves, in two phases (ncu r03c / r03d: a thread per (curve,
+// point) waited on the chain offsets -> order -> flux, and one point with two observations in a warp made the other
+// 31 lanes sit through its FP64 divisions and square root).
+//  1. A thread per point.  No observation: null for the G curves.  Exactly one observation and float32 data -- nearly
+//     every point at the native cadence -- is copied, G independent loads in flight: the FP64 sequence (w f)/w and
+//     sqrt(1/w), w = 1/e^2, lands within 2^-50 of f and e, which are float32 numbers, so rounding to float32 returns
+//     f and e themselves, for every finite f and every finite e > 0 (e^2 is exact in FP64 and neither overflows nor
+//     vanishes).  Every other point goes on a list in shared memory.
+//  2. The listed (point, curve) pairs are dealt out over all the threads, so the FP64 arithmetic runs in full warps.
+// float64 data always takes the arithmetic (it is not the identity there).
+template <typename T, int G>
+__global__ void __launch_bounds__(256) resample_sum_kernel(const T *__restrict__ flux, const T *__restrict__ flux_err,
+                                                           long long n_in, int n_lc, int n_out,
+                                                           const int *__restrict__ offsets,
+                                                           const int *__restrict__ order, T *__restrict__ flux_out,
+                                                           T *__restrict__ err_out) {
+    __shared__ int s_n;
+    __shared__ int s_point[256];
+    if (threadIdx.x == 0) s_n = 0;
+    __syncthreads();
+    const int c = blockIdx.x * 256 + threadIdx.x;
+    int lo = 0, m = -1;                                           // -1: past the last point
+    if (c < n_out) {
+        lo = offsets[c];
+        m = offsets[c + 1] - lo;
+    }
+    const bool copy = sizeof(T) == 4 && m == 1;
+    const int first = copy ? order[lo] : 0;
+    if (m > 0 && !copy) s_point[atomicAdd(&s_n, 1)] = c;
+    __syncthreads();
+    const int n_listed = s_n;
+    const T nan_t = static_cast<T>(__longlong_as_double(0x7ff8000000000000LL));
+    const T inf_t = static_cast<T>(__longlong_as_double(0x7ff0000000000000LL));
+    for (int lc0 = blockIdx.y * G; lc0 < n_lc; lc0 += gridDim.y * G) {
+        const int g_n = min(G, n_lc - lc0);
+        const T *fl = flux + static_cast<long long>(lc0) * n_in, *er = flux_err + static_cast<long long>(lc0) * n_in;
+        T *fo = flux_out + static_cast<long long>(lc0) * n_out, *eo = err_out + static_cast<long long>(lc0) * n_out;
+        if (copy) {
+            T f[G], e[G];
+#pragma unroll
+            for (int g = 0; g < G; ++g) {
+                f[g] = g < g_n ? fl[g * n_in + first] : T(0);
+                e[g] = g < g_n ? er[g * n_in + first] : T(0);
+            }
+#pragma unroll
+            for (int g = 0; g < G; ++g) {
+                if (g >= g_n) break;
+                const bool ok = isfinite(f[g]) && isfinite(e[g]) && e[g] > T(0);
+                fo[static_cast<long long>(g) * n_out + c] = ok ? f[g] : nan_t;
+                eo[static_cast<long long>(g) * n_out + c] = ok ? e[g] : inf_t;
+            }
+        } else if (m == 0) {
+            for (int g = 0; g < g_n; ++g) {
+                fo[static_cast<long long>(g) * n_out + c] = nan_t;
+                eo[static_cast<long long>(g) * n_out + c] = inf_t;
+            }
+        }
+        for (int task = threadIdx.x; task < n_listed * g_n; task += 256) {
+            const int g = task / n_listed, pc = s_point[task - g * n_listed];
+            const int plo = offsets[pc];
+            resample_point<T>(fl + g * n_in, er + g * n_in, order, plo, offsets[pc + 1] - plo,
+                              fo + static_cast<long long>(g) * n_out + pc, eo + static_cast<long long>(g) * n_out + pc);
         }
     }
 }
@@ -298,9 +525,12 @@ int cetra_resample_grid(const double *times_host, int64_t n, double cadence, dou
     return CETRA_OK;
 }
 
-size_t cetra_resample_workspace_bytes(int32_t n_lc, int64_t n_out) {
-    if (n_lc < 1 || n_out < 1) return 0;
-    return align_up(sizeof(double2) * static_cast<size_t>(n_lc) * static_cast<size_t>(n_out));
+size_t cetra_resample_workspace_bytes(int64_t n_in, int32_t n_lc, int64_t n_out) {
+    if (n_in < 0 || n_lc < 1 || n_out < 1 || n_in > 0x7fffffffLL || n_out > 0x7ffffffeLL) return 0;
+    // output point of every observation, its slot in the per-point lists, counts / cursors, offsets, scan tile totals
+    return 2 * align_up(sizeof(int) * static_cast<size_t>(std::max<int64_t>(n_in, 1))) +
+           align_up(sizeof(int) * static_cast<size_t>(n_out)) + align_up(sizeof(int) * static_cast<size_t>(n_out + 1)) +
+           align_up(sizeof(int) * static_cast<size_t>((n_out + kScanTile - 1) / kScanTile));
 }
 
 int cetra_resample(const double *times_dev, const void *flux_dev, const void *flux_err_dev, cetra_dtype dtype,
@@ -311,30 +541,44 @@ int cetra_resample(const double *times_dev, const void *flux_dev, const void *fl
         n_out < 1 || !(cadence > 0.0) || !std::isfinite(cadence) || !std::isfinite(t_start) ||
         (dtype != CETRA_F32 && dtype != CETRA_F64))
         return CETRA_ERR_INVALID_ARG;
-    if (!ws_ok(workspace_dev, workspace_bytes, cetra_resample_workspace_bytes(n_lc, n_out))) return CETRA_ERR_WORKSPACE;
+    if (n_in > 0x7fffffffLL || n_out > 0x7ffffffeLL) return CETRA_ERR_UNSUPPORTED;      // 32-bit indices
+    if (!ws_ok(workspace_dev, workspace_bytes, cetra_resample_workspace_bytes(n_in, n_lc, n_out)))
+        return CETRA_ERR_WORKSPACE;
     if (have_device() != CETRA_OK) return CETRA_ERR_CUDA;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    double2 *sums = static_cast<double2 *>(workspace_dev);
-    const long long total_out = static_cast<long long>(n_lc) * n_out;
-    CETRA_CUDA_TRY(cudaMemsetAsync(sums, 0, sizeof(double2) * static_cast<size_t>(total_out), st));
-    const long long total_in = static_cast<long long>(n_lc) * n_in;
-    if (total_in > 0) {
-        if (dtype == CETRA_F32)
-            resample_accumulate_kernel<float><<<stream_blocks(total_in), 256, 0, st>>>(
-                times_dev, static_cast<const float *>(flux_dev), static_cast<const float *>(flux_err_dev), n_in, n_lc,
-                t_start, cadence, n_out, sums);
-        else
-            resample_accumulate_kernel<double><<<stream_blocks(total_in), 256, 0, st>>>(
-                times_dev, static_cast<const double *>(flux_dev), static_cast<const double *>(flux_err_dev), n_in,
-                n_lc, t_start, cadence, n_out, sums);
+    Carver ws(workspace_dev);
+    int *cell_of = ws.take<int>(static_cast<size_t>(std::max<int64_t>(n_in, 1)));
+    int *order = ws.take<int>(static_cast<size_t>(std::max<int64_t>(n_in, 1)));
+    int *count = ws.take<int>(static_cast<size_t>(n_out));
+    int *offsets = ws.take<int>(static_cast<size_t>(n_out + 1));
+    int *tile_sum = ws.take<int>(static_cast<size_t>((n_out + kScanTile - 1) / kScanTile));
+    const int ni = static_cast<int>(n_in), no = static_cast<int>(n_out);
+    CETRA_CUDA_TRY(cudaMemsetAsync(count, 0, sizeof(int) * static_cast<size_t>(n_out), st));
+    if (n_in > 0) {
+        resample_cells_kernel<<<stream_blocks(n_in), 256, 0, st>>>(times_dev, ni, t_start, cadence, no, cell_of, count);
         CETRA_LAUNCH_CHECK();
     }
+    const int tiles = (no + kScanTile - 1) / kScanTile;
+    resample_tile_sums_kernel<<<tiles, kScanThreads, 0, st>>>(count, no, tile_sum);
+    CETRA_LAUNCH_CHECK();
+    resample_scan_kernel<<<tiles, kScanThreads, 0, st>>>(count, tile_sum, offsets, no);
+    CETRA_LAUNCH_CHECK();
+    if (n_in > 0) {
+        resample_fill_kernel<<<stream_blocks(n_in), 256, 0, st>>>(cell_of, ni, count, order);
+        CETRA_LAUNCH_CHECK();
+        resample_sort_kernel<<<stream_blocks(n_out), 256, 0, st>>>(offsets, no, order);
+        CETRA_LAUNCH_CHECK();
+    }
+    constexpr int kCurvesPerThread = 8;
+    const dim3 grid((no + 255) / 256, std::min((n_lc + kCurvesPerThread - 1) / kCurvesPerThread, 65535));
     if (dtype == CETRA_F32)
-        resample_finalize_kernel<float><<<stream_blocks(total_out), 256, 0, st>>>(
-            sums, total_out, static_cast<float *>(flux_out_dev), static_cast<float *>(flux_err_out_dev));
+        resample_sum_kernel<float, kCurvesPerThread><<<grid, 256, 0, st>>>(
+            static_cast<const float *>(flux_dev), static_cast<const float *>(flux_err_dev), n_in, n_lc, no, offsets,
+            order, static_cast<float *>(flux_out_dev), static_cast<float *>(flux_err_out_dev));
     else
-        resample_finalize_kernel<double><<<stream_blocks(total_out), 256, 0, st>>>(
-            sums, total_out, static_cast<double *>(flux_out_dev), static_cast<double *>(flux_err_out_dev));
+        resample_sum_kernel<double, kCurvesPerThread><<<grid, 256, 0, st>>>(
+            static_cast<const double *>(flux_dev), static_cast<const double *>(flux_err_dev), n_in, n_lc, no, offsets,
+            order, static_cast<double *>(flux_out_dev), static_cast<double *>(flux_err_out_dev));
     CETRA_LAUNCH_CHECK();
     return CETRA_OK;
 }

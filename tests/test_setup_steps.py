@@ -58,8 +58,11 @@ def test_setup_argument_errors_without_a_device(cetra):
     same = np.array([1.0, 1.0, 1.0])
     assert lib.cetra_median_cadence(same.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), 3,
                                     ctypes.byref(out)) == cetra.CETRA_ERR_INVALID_ARG
-    assert lib.cetra_resample_workspace_bytes(0, 10) == 0
-    assert lib.cetra_resample_workspace_bytes(2, 1000) >= 2 * 1000 * 16
+    assert lib.cetra_resample_workspace_bytes(100, 0, 10) == 0
+    assert lib.cetra_resample_workspace_bytes(3000, 2, 1000) >= 4 * (2 * 3000 + 2 * 1000 + 1)
+    # the lists are shared by the light curves: the scratch does not grow with their number
+    assert lib.cetra_resample_workspace_bytes(3000, 64, 1000) == lib.cetra_resample_workspace_bytes(3000, 2, 1000)
+    assert lib.cetra_resample_workspace_bytes(2 ** 31, 1, 1000) == 0           # 32-bit indices
     assert lib.cetra_monotransit_workspace_bytes(3, 1000) >= 3 * 1000 * 9
     assert lib.cetra_mask_workspace_bytes(5) >= 3 * 5 * 8
     # invalid arguments are reported before any device work
@@ -98,6 +101,34 @@ def test_resample_matches_oracle(dtype, shuffle, cad_factor, torch_cuda, cetra, 
     assert np.all(np.isnan(of[:, :pad_n])) and np.all(np.isnan(of[:, n_out - pad_n:]))
     if cad_factor >= 1.0:
         assert n_multi > 0                      # some points did combine several observations
+
+
+@pytest.mark.gpu
+def test_resample_sums_in_input_order_bit_for_bit(torch_cuda, cetra, oracle_mod):
+    """cetra_resample adds a point's observations in ascending input index in FP64, which is the order of the oracle's
+    sequential loop: in float64 the two are therefore bit-identical (not merely within rounding), also for shuffled
+    input and on a degenerate grid where thousands of observations share one output point (the heapsort branch of the
+    per-point index sort); and two runs give the same bits (no floating-point atomics)."""
+    from cetra_synth import make_irregular_batch
+    torch = torch_cuda
+    same = lambda a, b: np.array_equal(a, b, equal_nan=True)
+    for shuffle, cad_factor in ((True, 1.0), (False, 3.7), (True, 40.0)):
+        t, f, e = make_irregular_batch(n_lc=2, n=5000, dtype=np.float64, shuffle=shuffle)
+        t_start, c, n_out = cetra.cetra_resample_grid(t, cad_factor * cetra.cetra_median_cadence(t), 0.1)
+        dev = [torch.from_numpy(a).cuda() for a in (t, f, e)]
+        first = [a.cpu().numpy() for a in cetra.cetra_resample(*dev, t_start, c, n_out)]
+        again = [a.cpu().numpy() for a in cetra.cetra_resample(*dev, t_start, c, n_out)]
+        assert same(first[0], again[0]) and same(first[1], again[1])
+        for b in range(2):
+            rf, re = oracle_mod.resample(t, f[b], e[b], t_start, c, n_out)
+            assert same(first[0][b], rf) and same(first[1][b], re), (shuffle, cad_factor, b)
+    # everything in three points: lists of thousands of indices
+    t, f, e = make_irregular_batch(n_lc=1, n=20000, dtype=np.float64, shuffle=True)
+    span = t.max() - t.min()
+    of, oe = cetra.cetra_resample(torch.from_numpy(t).cuda(), torch.from_numpy(f).cuda(), torch.from_numpy(e).cuda(),
+                                  t.min(), span / 2.0, 3)
+    rf, re = oracle_mod.resample(t, f[0], e[0], t.min(), span / 2.0, 3)
+    assert same(of.cpu().numpy()[0], rf) and same(oe.cpu().numpy()[0], re)
 
 
 @pytest.mark.gpu
