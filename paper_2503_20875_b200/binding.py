@@ -34,13 +34,17 @@ EXPORTED_SYMBOLS = (
     "cetra_search_batched_workspace_bytes", "cetra_search_batched", "cetra_search_batched_templates",
     "cetra_search_batched_templates_workspace_bytes",
     "cetra_search_batched_host_workspace_bytes", "cetra_search_batched_host",
-    "cetra_profile_enable", "cetra_profile_read", "cetra_peak_probe_workspace_bytes", "cetra_peak_probe",
-    "cetra_tc_correlation_probe_workspace_bytes", "cetra_tc_correlation_probe",
+    "cetra_profile_enable", "cetra_profile_read",
     "cetra_resample_template", "cetra_median_cadence", "cetra_resample_grid", "cetra_resample_workspace_bytes", "cetra_resample",
     "cetra_resample_static_max_points", "cetra_resample_static", "cetra_test_fold_override",
     "cetra_monotransit_workspace_bytes", "cetra_monotransit_search",
     "cetra_mask_workspace_bytes", "cetra_mask_transits",
 )
+
+
+# The probes of include/cetra_diag.h, exported by libcetra_diag.so only.
+DIAG_SYMBOLS = ("cetra_peak_probe_workspace_bytes", "cetra_peak_probe",
+                "cetra_tc_correlation_probe_workspace_bytes", "cetra_tc_correlation_probe")
 
 
 class CetraError(RuntimeError):
@@ -154,11 +158,29 @@ def load_library() -> ctypes.CDLL:
     lib.cetra_profile_enable.argtypes = [i32]
     lib.cetra_profile_read.restype = ctypes.c_int
     lib.cetra_profile_read.argtypes = [dp, ctypes.POINTER(i64), dp, ctypes.POINTER(i64), i32]
+    _lib = lib
+    return lib
+
+
+_diag: Optional[ctypes.CDLL] = None
+
+
+def load_diag_library() -> ctypes.CDLL:
+    """dlopen libcetra_diag.so, the measurement probes (include/cetra_diag.h); built on demand like the product."""
+    global _diag
+    if _diag is not None:
+        return _diag
+    path = _build.DIAG_LIB_PATH
+    if not os.path.exists(path) or (_build.stale(path) and _build.have_nvcc()):
+        path = _build.build_diag()
+    lib = ctypes.CDLL(path)
+    vp, dp = ctypes.c_void_p, ctypes.POINTER(ctypes.c_double)
+    i32, sz = ctypes.c_int32, ctypes.c_size_t
     lib.cetra_peak_probe_workspace_bytes.restype = sz
     lib.cetra_peak_probe_workspace_bytes.argtypes = []
     lib.cetra_peak_probe.restype = ctypes.c_int
     lib.cetra_peak_probe.argtypes = [i32, i32, dp, dp, vp, sz, vp]
-    _lib = lib
+    _diag = lib
     return lib
 
 
@@ -294,9 +316,10 @@ CETRA_PROBE_FFMA2, CETRA_PROBE_FADD2, CETRA_PROBE_LDS64 = 0, 1, 2
 
 @_on_stream
 def cetra_peak_probe(kind: int, iters: int = 20000, stream=None):
-    """(units per clock per SM, units per second) of one of the probed instructions; synchronises the stream."""
+    """(units per clock per SM, units per second) of one of the probed instructions; synchronises the stream.
+    A probe of libcetra_diag.so (include/cetra_diag.h), not of the product library."""
     torch = _torch()
-    lib = load_library()
+    lib = load_diag_library()
     nbytes = int(lib.cetra_peak_probe_workspace_bytes())
     ws = _workspace(torch, nbytes, torch.device("cuda", torch.cuda.current_device()))
     a, b = ctypes.c_double(), ctypes.c_double()
@@ -307,9 +330,9 @@ def cetra_peak_probe(kind: int, iters: int = 20000, stream=None):
 
 @_on_stream
 def cetra_tc_correlation_probe(n_out: int, n_taps: int, split: bool = True, reps: int = 20, stream=None):
-    """The measured tensor-core variant of the windowed sums (cetra.h): dict(ms, evals_per_s, err_wmf, err_wmm)."""
+    """The measured tensor-core variant of the windowed sums (cetra_diag.h): dict(ms, evals_per_s, err_wmf, err_wmm)."""
     torch = _torch()
-    lib = load_library()
+    lib = load_diag_library()
     lib.cetra_tc_correlation_probe_workspace_bytes.restype = ctypes.c_size_t
     lib.cetra_tc_correlation_probe_workspace_bytes.argtypes = [ctypes.c_int64, ctypes.c_int32]
     lib.cetra_tc_correlation_probe.restype = ctypes.c_int

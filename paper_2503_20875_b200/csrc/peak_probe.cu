@@ -13,8 +13,13 @@
 #include <vector>
 
 #include "common.cuh"
+#include "cetra_diag.h"
 
 namespace cetra {
+
+// libcetra_diag.so is linked on its own: it keeps a launch counter of its own (the product's counts only the
+// product's kernels).
+std::atomic<int64_t> g_launch_count{0};
 
 namespace {
 

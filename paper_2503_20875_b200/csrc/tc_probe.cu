@@ -15,6 +15,7 @@
 #include <vector>
 
 #include "common.cuh"
+#include "cetra_diag.h"
 
 namespace cetra {
 

@@ -30,6 +30,14 @@ def test_library_exports_every_declared_symbol(cetra):
     lib = cetra.load_library()
     for name in declared:
         assert getattr(lib, name) is not None
+    # the measurement probes have a header and a library of their own; the product exports none of them
+    diag_header = open(os.path.join(ROOT, "include", "cetra_diag.h")).read()
+    diag_declared = set(re.findall(r"\b(cetra_[a-z0-9_]+)\s*\(", diag_header))
+    assert diag_declared == set(cetra.DIAG_SYMBOLS) and not (diag_declared & declared)
+    diag = cetra.load_diag_library()
+    for name in diag_declared:
+        assert getattr(diag, name) is not None
+        assert not hasattr(lib, name), f"{name} leaked into the product ABI"
 
 
 def test_product_does_not_import_the_oracle():
